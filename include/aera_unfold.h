@@ -1,0 +1,165 @@
+/*
+ * aera_unfold.h -- C ABI of the B200-native per-station E-field unfolding library
+ * (libaera_unfold.so), the data-parallel hot path of the AERA radio reconstruction of
+ * arXiv 1507.07733.
+ *
+ * The operation (section 2: "the antenna pattern for this direction is evaluated,
+ * and the E-field trace at each station reconstructed from the voltage traces. Finally, the
+ * maximum of the envelope of the E-field trace is used as updated timing information";
+ * section 3: vector effective length tabulated on (frequency, zenith, azimuth) nodes and
+ * interpolated linearly; section 4, L59-63 and L71: Fourier transforms and the Hilbert envelope):
+ *
+ *   for every station of every event, with the event's shower direction (theta, phi):
+ *     V_c[k]  = sum_n v_c[n] exp(-2 pi i n k / N)              c = 0,1  (forward real DFT)
+ *     H_cp[k] = trilinear interpolation of the tabulated complex response at
+ *               (theta, phi, f_k = k fs / N); azimuth periodic; bins outside the table
+ *               band, DC and Nyquist are zeroed
+ *     E[k]    = H[k]^-1 V[k]                                   (2x2 complex solve, p = theta,phi)
+ *     z_p[n]  = (2/N) sum_{k in band} E_p[k] exp(+2 pi i n k / N)   (analytic signal)
+ *     e_p[n]  = Re z_p[n]                                      (E-field traces)
+ *     env[n]  = sqrt(|z_theta[n]|^2 + |z_phi[n]|^2)            (Hilbert envelope)
+ *     peak_amp = max_n env[n], peak_idx = smallest n attaining it
+ *
+ * All entry points are plain C: pointers (host or device as stated per argument), sizes,
+ * and an opaque CUDA stream handle (cudaStream_t passed as void*; NULL = legacy default
+ * stream).  No exceptions cross the ABI; every call returns an aera_status_t and sets a
+ * thread-local message readable with aera_last_error().
+ *
+ * Unless stated otherwise calls are ASYNCHRONOUS on the given stream: they validate their
+ * arguments on the host, enqueue kernels, and return without synchronising.  They allocate
+ * nothing on the hot path: scratch memory is caller-provided (aera_workspace_bytes).  The only
+ * allocations the library makes are (a) inside aera_pattern_upload, (b) the first time a
+ * pattern is used with a new (n_samples, fs_hz) pair, when a small plan (twiddle tables,
+ * per-bin frequency cell/weight table) is built and cached in the pattern handle -- that first
+ * call synchronises the stream once -- and (c) inside the *_host convenience entry point.
+ */
+#ifndef AERA_UNFOLD_H
+#define AERA_UNFOLD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct aera_pattern aera_pattern_t; /* opaque; owns the device copy of one table + plans */
+
+typedef enum { AERA_F32 = 0, AERA_F64 = 1 } aera_dtype_t;
+
+typedef enum {
+    AERA_OK = 0,
+    AERA_ERR_INVALID_ARG = 1,   /* NULL pointer, non-positive size, misaligned buffer, bad grid */
+    AERA_ERR_UNSUPPORTED_N = 2, /* n_samples not a power of two in [64, 65536] */
+    AERA_ERR_DTYPE_MISMATCH = 3,/* dtype differs from the pattern's dtype */
+    AERA_ERR_WORKSPACE = 4,     /* workspace NULL/misaligned/smaller than aera_workspace_bytes() */
+    AERA_ERR_ALLOC = 5,         /* cudaMalloc / host allocation failed */
+    AERA_ERR_CUDA = 6,          /* a CUDA runtime call or launch failed; message has the string */
+    AERA_ERR_BAND = 7           /* table band does not lie inside (0, fs/2) or contains no bin */
+} aera_status_t;
+
+/* Uniform node grids. Angles in DEGREES, frequency in Hz ("discrete frequencies and
+ * zenith and azimuth angles").  When azimuth_periodic != 0 the axis has period
+ * (n_azimuth-1)*dazimuth_deg and the stored last node must duplicate the first; the library never
+ * reads the last node and wraps instead.  Zenith outside the table is clamped to the table. */
+typedef struct {
+    int dtype;              /* AERA_F32: complex64 table; AERA_F64: complex128 table */
+    int n_zenith;  double zenith0_deg,  dzenith_deg;    /* >= 2 nodes, step > 0 */
+    int n_azimuth; double azimuth0_deg, dazimuth_deg;   /* >= 2 nodes (>= 3 if periodic), step > 0 */
+    int azimuth_periodic;
+    int n_freq;    double freq0_hz, dfreq_hz;           /* 2 <= n_freq <= 512, step > 0 */
+} aera_pattern_desc_t;
+
+/* Copy one antenna-response table to the device and repack it (once) into the library's
+ * layout [zenith][azimuth][freq][channel*2+pol] ("the patterns are copied and
+ * converted ... only once on first access").
+ *   H    interleaved (re, im), C order [channel 2][pol 2 (theta,phi)][n_zenith][n_azimuth][n_freq],
+ *        element type complex64 or complex128 per desc->dtype.  HOST pointer if
+ *        src_on_device == 0, DEVICE pointer otherwise.  Not retained: the caller may free it
+ *        after the call returns (the call synchronises the stream before returning).
+ *   out  receives the handle; release with aera_pattern_free. Several patterns may be resident.
+ * Errors: INVALID_ARG (NULL, bad grid), ALLOC, CUDA. */
+aera_status_t aera_pattern_upload(const aera_pattern_desc_t *desc, const void *H, int src_on_device,
+                                  void *cuda_stream, aera_pattern_t **out);
+
+/* Frees the device table and all cached plans. The caller guarantees no kernel using it is in
+ * flight. NULL is accepted. */
+aera_status_t aera_pattern_free(aera_pattern_t *pattern);
+
+/* In-band DFT bins for (pattern, n_samples, fs_hz): k_lo..k_hi inclusive, the bins with
+ * freq0 <= k*fs/N <= freq0+(n_freq-1)*dfreq and 0 < k < N/2 (evaluated exactly in integers when
+ * fs, freq0, dfreq are whole numbers of Hz).  Errors: UNSUPPORTED_N, BAND. */
+aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_hz,
+                        int *k_lo, int *k_hi);
+
+typedef enum { AERA_OP_UNFOLD = 0, AERA_OP_SCAN = 1 } aera_op_t;
+
+/* Scratch bytes needed by aera_unfold_batch (n_events_or_dirs = n_events) or
+ * aera_scan_directions (n_events_or_dirs = n_dirs) for these sizes; 0 on invalid arguments
+ * (aera_last_error tells why).  The workspace holds the per-event (per-direction) inverse
+ * response matrices and, for the kernels that need it, per-CTA transform buffers / per-station
+ * spectra.  Contents are undefined between calls; one workspace must not be shared by calls
+ * that may run concurrently. */
+size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dtype,
+                            long n_events_or_dirs, int n_stations, int n_samples, double fs_hz);
+
+/* Batched unfolding (PAPER.md L29 step 3+4 for every station of every event).
+ *   traces    DEVICE [n_events][n_stations][2 channels][n_samples] real (dtype), 16-byte aligned
+ *   dirs      DEVICE [n_events][2] double: (zenith_deg, azimuth_deg), one direction per event
+ *   efield    DEVICE [n_events][n_stations][2 (theta,phi)][n_samples] real (dtype), 16-byte aligned;
+ *             may be the same pointer as traces (in place); may be NULL (peaks only)
+ *   peak_amp  DEVICE [n_events][n_stations] real (dtype)     envelope maximum
+ *   peak_idx  DEVICE [n_events][n_stations] int32            smallest sample index attaining it
+ *   workspace DEVICE, 256-byte aligned, >= aera_workspace_bytes(AERA_OP_UNFOLD, ...)
+ * All buffers are caller-owned. n_samples: power of two in [64, 65536]. The result is linear in
+ * the traces; units are the caller's (configs: microvolt in, microvolt/metre out).
+ * NaN/Inf in the data are not checked (they propagate). n_events == 0 is a no-op.
+ * Errors: INVALID_ARG, UNSUPPORTED_N, DTYPE_MISMATCH, WORKSPACE, BAND, ALLOC (first-use plan), CUDA. */
+aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                int n_samples, double fs_hz, const void *traces, const double *dirs,
+                                void *efield, void *peak_amp, int32_t *peak_idx,
+                                void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Direction-hypothesis scan (BASELINE configs[2]; motivated by PAPER.md L29: the pattern is
+ * re-evaluated at a new direction in every iteration of the reconstruction loop): one forward
+ * transform per station, then unfolding + envelope peak at every direction; no trace output.
+ *   traces    DEVICE [n_stations][2][n_samples] real (dtype), 16-byte aligned
+ *   dirs      DEVICE [n_dirs][2] double (zenith_deg, azimuth_deg)
+ *   peak_amp  DEVICE [n_dirs][n_stations] real (dtype);  peak_idx DEVICE [n_dirs][n_stations] int32
+ *   workspace DEVICE, 256-byte aligned, >= aera_workspace_bytes(AERA_OP_SCAN, ..., n_dirs, ...)
+ * Errors as aera_unfold_batch. */
+aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int n_stations,
+                                   int n_samples, double fs_hz, const void *traces,
+                                   long n_dirs, const double *dirs,
+                                   void *peak_amp, int32_t *peak_idx,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* End-to-end convenience for HOST buffers (the paper's situation: traces live on
+ * the host and are copied for every transform).  Same arguments as aera_unfold_batch but every
+ * data pointer is a HOST pointer (page-locked memory gives full PCIe speed; pageable works).
+ * The batch is cut into event chunks that flow through a 3-stream pipeline
+ * (H2D copy | unfold kernels | D2H copy) over device staging buffers owned by the pattern handle
+ * (allocated on first use, reused afterwards).  SYNCHRONOUS: results are in the host buffers on
+ * return.  efield may be NULL. */
+aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                     int n_samples, double fs_hz, const void *traces_host,
+                                     const double *dirs_host, void *efield_host, void *peak_amp_host,
+                                     int32_t *peak_idx_host);
+
+/* Kernel selection, for tests and tuning. 0 = automatic (specialised kernels where available),
+ * 1 = always the generic radix-2 kernel. Process-wide. Returns the previous value. */
+int aera_set_kernel_variant(int variant);
+
+/* Number of kernel launches this library has enqueued since load (monotonic, all threads). */
+unsigned long long aera_launch_count(void);
+
+/* Message for the most recent non-OK status on this thread ("" if none). Static storage. */
+const char *aera_last_error(void);
+
+/* Library version string, e.g. "aera_unfold 0.1 (sm_100a)". */
+const char *aera_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AERA_UNFOLD_H */

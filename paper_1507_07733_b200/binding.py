@@ -1,0 +1,236 @@
+"""ctypes binding of libaera_unfold.so -- argument marshalling only.
+
+Function names and argument order mirror include/aera_unfold.h. torch is used for device
+memory and streams, nothing else: every step of the path runs in the library's kernels.
+Raises ImportError if the library cannot be built/loaded (no fallback of any kind).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+AERA_F32, AERA_F64 = 0, 1
+AERA_OP_UNFOLD, AERA_OP_SCAN = 0, 1
+STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 3: "AERA_ERR_DTYPE_MISMATCH",
+          4: "AERA_ERR_WORKSPACE", 5: "AERA_ERR_ALLOC", 6: "AERA_ERR_CUDA", 7: "AERA_ERR_BAND"}
+
+EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
+           "aera_scan_directions", "aera_unfold_batch_host", "aera_set_kernel_variant", "aera_launch_count",
+           "aera_last_error", "aera_version")
+
+
+class AeraError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class PatternDesc(C.Structure):
+    _fields_ = [
+        ("dtype", C.c_int),
+        ("n_zenith", C.c_int), ("zenith0_deg", C.c_double), ("dzenith_deg", C.c_double),
+        ("n_azimuth", C.c_int), ("azimuth0_deg", C.c_double), ("dazimuth_deg", C.c_double),
+        ("azimuth_periodic", C.c_int),
+        ("n_freq", C.c_int), ("freq0_hz", C.c_double), ("dfreq_hz", C.c_double),
+    ]
+
+
+def _load():
+    try:
+        path = _build.build()
+    except Exception as e:  # no nvcc and no prebuilt library
+        if os.path.exists(_build.LIB):
+            path = _build.LIB
+        else:
+            raise ImportError(f"libaera_unfold.so is missing and could not be built: {e}") from e
+    try:
+        lib = C.CDLL(path)
+    except OSError as e:
+        raise ImportError(f"cannot load {path}: {e}") from e
+    vp, ip, dp = C.c_void_p, C.POINTER(C.c_int), C.c_void_p
+    lib.aera_pattern_upload.argtypes = [C.POINTER(PatternDesc), vp, C.c_int, vp, C.POINTER(vp)]
+    lib.aera_pattern_upload.restype = C.c_int
+    lib.aera_pattern_free.argtypes = [vp]
+    lib.aera_pattern_free.restype = C.c_int
+    lib.aera_band.argtypes = [vp, C.c_int, C.c_double, ip, ip]
+    lib.aera_band.restype = C.c_int
+    lib.aera_workspace_bytes.argtypes = [C.c_int, vp, C.c_int, C.c_long, C.c_int, C.c_int, C.c_double]
+    lib.aera_workspace_bytes.restype = C.c_size_t
+    lib.aera_unfold_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.aera_unfold_batch.restype = C.c_int
+    lib.aera_scan_directions.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, vp, C.c_long, dp, vp, vp, vp, C.c_size_t, vp]
+    lib.aera_scan_directions.restype = C.c_int
+    lib.aera_unfold_batch_host.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp]
+    lib.aera_unfold_batch_host.restype = C.c_int
+    lib.aera_set_kernel_variant.argtypes = [C.c_int]
+    lib.aera_set_kernel_variant.restype = C.c_int
+    lib.aera_launch_count.restype = C.c_ulonglong
+    lib.aera_last_error.restype = C.c_char_p
+    lib.aera_version.restype = C.c_char_p
+    return lib, path
+
+
+_lib, LIBRARY_PATH = _load()
+
+
+def _check(st):
+    if st != 0:
+        raise AeraError(st, _lib.aera_last_error().decode())
+
+
+def _dtype_code(t: torch.dtype) -> int:
+    if t in (torch.float32, torch.complex64):
+        return AERA_F32
+    if t in (torch.float64, torch.complex128):
+        return AERA_F64
+    raise TypeError(f"unsupported dtype {t}")
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+class Pattern:
+    """Owner of an aera_pattern_t handle."""
+
+    def __init__(self, handle, desc: PatternDesc):
+        self.handle = handle
+        self.desc = desc
+        self.dtype = desc.dtype
+
+    def free(self):
+        if self.handle:
+            _lib.aera_pattern_free(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def make_desc(grid, dtype_code: int) -> PatternDesc:
+    """grid: any object with the PatternGrid attribute names of aera_inputs."""
+    return PatternDesc(dtype_code, grid.n_zenith, grid.zenith0_deg, grid.dzenith_deg, grid.n_azimuth, grid.azimuth0_deg,
+                       grid.dazimuth_deg, 1 if grid.azimuth_periodic else 0, grid.n_freq, grid.freq0_hz, grid.dfreq_hz)
+
+
+def aera_version() -> str:
+    return _lib.aera_version().decode()
+
+
+def aera_launch_count() -> int:
+    return int(_lib.aera_launch_count())
+
+
+def aera_set_kernel_variant(variant: int) -> int:
+    return int(_lib.aera_set_kernel_variant(int(variant)))
+
+
+def aera_pattern_upload(desc: PatternDesc, H, stream=None) -> Pattern:
+    """H: numpy complex array (host) or torch CUDA complex tensor, shape [2][2][n_z][n_a][n_f]."""
+    shape = (2, 2, desc.n_zenith, desc.n_azimuth, desc.n_freq)
+    want = np.complex64 if desc.dtype == AERA_F32 else np.complex128
+    handle = C.c_void_p()
+    if isinstance(H, torch.Tensor):
+        if tuple(H.shape) != shape or _dtype_code(H.dtype) != desc.dtype or not H.is_contiguous():
+            raise ValueError("H must be a contiguous tensor of shape [2][2][n_z][n_a][n_f] in the descriptor's dtype")
+        on_dev = 1 if H.is_cuda else 0
+        st = _lib.aera_pattern_upload(C.byref(desc), _ptr(H), on_dev, _stream_ptr(stream), C.byref(handle))
+    else:
+        Hn = np.ascontiguousarray(H)
+        if Hn.shape != shape or Hn.dtype != want:
+            raise ValueError(f"H must have shape {shape} and dtype {want}")
+        st = _lib.aera_pattern_upload(C.byref(desc), C.c_void_p(Hn.ctypes.data), 0, _stream_ptr(stream), C.byref(handle))
+    _check(st)
+    return Pattern(handle, desc)
+
+
+def aera_pattern_free(p: Pattern):
+    p.free()
+
+
+def aera_band(p: Pattern, n_samples: int, fs_hz: float):
+    lo, hi = C.c_int(), C.c_int()
+    _check(_lib.aera_band(p.handle, n_samples, fs_hz, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def aera_workspace_bytes(op: int, p: Pattern, dtype: int, n_events_or_dirs: int, n_stations: int, n_samples: int, fs_hz: float) -> int:
+    n = int(_lib.aera_workspace_bytes(op, p.handle, dtype, n_events_or_dirs, n_stations, n_samples, fs_hz))
+    if n == 0:
+        raise AeraError(1, _lib.aera_last_error().decode())
+    return n
+
+
+def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def aera_unfold_batch(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, efield=None, peak_amp=None,
+                      peak_idx=None, workspace=None, stream=None, want_efield=True):
+    """traces [E][S][2][N] CUDA real tensor, dirs [E][2] CUDA float64. Returns (efield|None, peak_amp, peak_idx)."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    if efield is None and want_efield:
+        efield = torch.empty_like(traces)
+    if peak_amp is None:
+        peak_amp = torch.empty((E, S), dtype=traces.dtype, device=traces.device)
+    if peak_idx is None:
+        peak_idx = torch.empty((E, S), dtype=torch.int32, device=traces.device)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, traces.device)
+    _check(_lib.aera_unfold_batch(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp),
+                                  _ptr(peak_idx), _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return efield, peak_amp, peak_idx
+
+
+def aera_scan_directions(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, peak_amp=None, peak_idx=None,
+                         workspace=None, stream=None):
+    """traces [S][2][N] CUDA, dirs [D][2] CUDA float64. Returns (peak_amp [D][S], peak_idx [D][S])."""
+    S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    D = dirs.shape[0]
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (D, 2) and dirs.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    if peak_amp is None:
+        peak_amp = torch.empty((D, S), dtype=traces.dtype, device=traces.device)
+    if peak_idx is None:
+        peak_idx = torch.empty((D, S), dtype=torch.int32, device=traces.device)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_SCAN, p, dt, D, S, N, fs_hz) if D > 0 else 256, traces.device)
+    _check(_lib.aera_scan_directions(p.handle, dt, S, N, fs_hz, _ptr(traces), D, _ptr(dirs), _ptr(peak_amp), _ptr(peak_idx),
+                                     _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return peak_amp, peak_idx
+
+
+def aera_unfold_batch_host(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, efield=None, peak_amp=None,
+                           peak_idx=None, want_efield=True):
+    """HOST tensors (pinned for full speed). Synchronous. Returns (efield|None, peak_amp, peak_idx) on the host."""
+    E, S, two, N = traces.shape
+    assert two == 2 and (not traces.is_cuda) and traces.is_contiguous()
+    assert (not dirs.is_cuda) and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    pin = traces.is_pinned()
+    if efield is None and want_efield:
+        efield = torch.empty(traces.shape, dtype=traces.dtype, pin_memory=pin)
+    if peak_amp is None:
+        peak_amp = torch.empty((E, S), dtype=traces.dtype, pin_memory=pin)
+    if peak_idx is None:
+        peak_idx = torch.empty((E, S), dtype=torch.int32, pin_memory=pin)
+    _check(_lib.aera_unfold_batch_host(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp), _ptr(peak_idx)))
+    return efield, peak_amp, peak_idx

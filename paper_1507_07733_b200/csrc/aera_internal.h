@@ -1,0 +1,52 @@
+// Internal declarations shared by the translation units of libaera_unfold.so.
+// Nothing here is part of the C ABI (include/aera_unfold.h) and nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/aera_unfold.h"
+
+namespace aera {
+
+template <typename T> struct cx { T re, im; };
+
+// Geometry of the repacked table [n_z][n_a][n_f][4] (4 = channel*2 + pol).
+struct TableGeom {
+    int n_z, n_a, n_f, periodic;
+    double z0, dz, a0, da;
+};
+
+// Everything a kernel needs to know about one (pattern, N, fs) combination. Device pointers are
+// owned by the pattern handle (built on first use, see api.cu).
+struct PlanDev {
+    int N, logN;
+    int k_lo, k_hi, K;
+    const int *bin_if;      // [K] lower frequency node of bin k_lo+j
+    const double *bin_tf;   // [K] weight of the upper node
+    const void *tw;         // [N/2] cx<T>: W_N^m = exp(-2 pi i m / N), m < N/2 (generic kernel)
+    const void *tw1024;     // [1024] cx<T>: W_1024^m (warp kernels: 32x32 inter-pass twiddles)
+    const void *twN;        // [N] cx<T>: W_N^m, m < N (real-FFT split / polyphase twiddles)
+};
+
+void count_launches(unsigned n);
+int kernel_variant();
+
+// ---- pattern.cu
+cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);
+// Minv[d][j][4] = (2/N) * H(theta_d, phi_d, f_{k_lo+j})^-1, rows (theta0, theta1, phi0, phi1).
+cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
+                        const double *dirs, long n_dirs, void *minv, cudaStream_t s);
+size_t minv_smem_bytes(int dtype, int n_f);
+
+// ---- unfold_generic.cu
+size_t generic_scratch_bytes(int dtype, int N, long n_units);   // per-call global transform buffers (0 if smem-resident)
+cudaError_t launch_unfold_generic(int dtype, const PlanDev &p, long n_events, int n_stations,
+                                  const void *traces, void *efield, void *amp, int32_t *idx,
+                                  const void *minv, void *scratch, cudaStream_t s);
+size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations);
+cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, const void *traces,
+                                long n_dirs, const void *minv, void *amp, int32_t *idx,
+                                void *spectra, void *scratch, cudaStream_t s);
+
+} // namespace aera

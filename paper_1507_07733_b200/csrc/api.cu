@@ -1,0 +1,460 @@
+// C ABI of libaera_unfold.so (include/aera_unfold.h): argument validation, pattern handles,
+// plan cache, workspace layout, kernel dispatch, and the host-buffer pipeline.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <new>
+#include <utility>
+#include <vector>
+
+#include "aera_internal.h"
+
+namespace aera {
+
+static std::atomic<unsigned long long> g_launches{0};
+static std::atomic<int> g_variant{0};
+void count_launches(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+int kernel_variant() { return g_variant.load(std::memory_order_relaxed); }
+
+static thread_local char g_err[512] = "";
+
+static aera_status_t fail(aera_status_t st, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+static aera_status_t cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(AERA_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+struct Plan {
+    PlanDev dev{};
+    double fs = 0;
+    void *blob = nullptr; // one device allocation holding every table of the plan
+};
+
+struct HostPipe { // staging for aera_unfold_batch_host
+    cudaStream_t st[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_k[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    void *d_in[2] = {nullptr, nullptr}, *d_out[2] = {nullptr, nullptr}, *d_amp[2] = {nullptr, nullptr};
+    int32_t *d_idx[2] = {nullptr, nullptr};
+    double *d_dirs[2] = {nullptr, nullptr};
+    void *d_ws[2] = {nullptr, nullptr};
+    size_t cap_units = 0, cap_trace_bytes = 0, cap_ws = 0, cap_events = 0;
+    bool ready = false;
+};
+
+} // namespace aera
+
+using namespace aera;
+
+struct aera_pattern {
+    aera_pattern_desc_t desc{};
+    void *d_table = nullptr;
+    size_t table_bytes = 0;
+    std::mutex mu;
+    std::map<std::pair<int, double>, Plan *> plans;
+    HostPipe pipe;
+};
+
+namespace {
+
+const size_t kAlign = 256;
+size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+size_t real_bytes(int dtype) { return dtype == AERA_F32 ? 4 : 8; }
+size_t cplx_bytes(int dtype) { return 2 * real_bytes(dtype); }
+
+bool is_whole(double x) { return x == std::floor(x) && std::fabs(x) < 9.0e15; }
+
+int ilog2(int n)
+{
+    int l = 0;
+    while ((1 << l) < n) ++l;
+    return l;
+}
+
+aera_status_t check_n(int n_samples)
+{
+    if (n_samples < 64 || n_samples > 65536 || (n_samples & (n_samples - 1)) != 0)
+        return fail(AERA_ERR_UNSUPPORTED_N, "n_samples=%d is not a power of two in [64, 65536]", n_samples);
+    return AERA_OK;
+}
+
+// In-band bins: ceil(f0 N / fs) .. floor(f_hi N / fs), exact in integers for whole-Hz inputs.
+aera_status_t compute_band(const aera_pattern_desc_t &d, int N, double fs, int *k_lo, int *k_hi)
+{
+    if (!(fs > 0) || !std::isfinite(fs)) return fail(AERA_ERR_INVALID_ARG, "fs_hz must be positive and finite");
+    const double f_hi = d.freq0_hz + (d.n_freq - 1) * d.dfreq_hz;
+    if (!(d.freq0_hz > 0) || !(f_hi < 0.5 * fs))
+        return fail(AERA_ERR_BAND, "table band [%g, %g] Hz must lie strictly inside (0, fs/2 = %g)", d.freq0_hz, f_hi, 0.5 * fs);
+    long long lo, hi;
+    if (is_whole(fs) && is_whole(d.freq0_hz) && is_whole(d.dfreq_hz)) {
+        const __int128 F = (long long)fs;
+        const __int128 a = (__int128)(long long)d.freq0_hz * N;
+        const __int128 b = ((__int128)(long long)d.freq0_hz + (__int128)(d.n_freq - 1) * (long long)d.dfreq_hz) * N;
+        lo = (long long)((a + F - 1) / F);
+        hi = (long long)(b / F);
+    } else {
+        lo = (long long)std::ceil((long double)d.freq0_hz * N / (long double)fs);
+        hi = (long long)std::floor(((long double)d.freq0_hz + (long double)(d.n_freq - 1) * d.dfreq_hz) * N / (long double)fs);
+    }
+    if (lo < 1) lo = 1;
+    if (hi > N / 2 - 1) hi = N / 2 - 1;
+    if (hi < lo) return fail(AERA_ERR_BAND, "no DFT bin of N=%d, fs=%g falls inside the table band", N, fs);
+    *k_lo = (int)lo;
+    *k_hi = (int)hi;
+    return AERA_OK;
+}
+
+template <typename T>
+void fill_twiddles(cx<T> *dst, int count, int N)
+{
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < count; ++m) {
+        long double a = two_pi * (long double)m / (long double)N;
+        dst[m].re = (T)cosl(a);
+        dst[m].im = (T)(-sinl(a));
+    }
+}
+
+// Build (or fetch) the plan for (N, fs). May allocate and synchronise `s` on first use.
+aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan **out)
+{
+    std::lock_guard<std::mutex> lk(pat->mu);
+    auto key = std::make_pair(N, fs);
+    auto it = pat->plans.find(key);
+    if (it != pat->plans.end()) { *out = it->second; return AERA_OK; }
+
+    int k_lo, k_hi;
+    aera_status_t st = compute_band(pat->desc, N, fs, &k_lo, &k_hi);
+    if (st != AERA_OK) return st;
+    const int K = k_hi - k_lo + 1;
+    const int dtype = pat->desc.dtype;
+    const size_t cb = cplx_bytes(dtype);
+
+    // blob layout: bin_if [K] | bin_tf [K] | tw [N/2] | tw1024 [1024] | twN [N]
+    size_t off_if = 0;
+    size_t off_tf = align_up(off_if + sizeof(int) * K);
+    size_t off_tw = align_up(off_tf + sizeof(double) * K);
+    size_t off_t1k = align_up(off_tw + cb * (N / 2));
+    size_t off_twN = align_up(off_t1k + cb * 1024);
+    size_t total = align_up(off_twN + cb * N);
+    std::vector<unsigned char> h(total, 0);
+    int *bin_if = reinterpret_cast<int *>(h.data() + off_if);
+    double *bin_tf = reinterpret_cast<double *>(h.data() + off_tf);
+    for (int j = 0; j < K; ++j) {
+        const double f = (double)(k_lo + j) * fs / (double)N;
+        const double u = (f - pat->desc.freq0_hz) / pat->desc.dfreq_hz;
+        int i = (int)std::floor(u);
+        if (i > pat->desc.n_freq - 2) i = pat->desc.n_freq - 2;
+        if (i < 0) i = 0;
+        bin_if[j] = i;
+        bin_tf[j] = u - (double)i;
+    }
+    if (dtype == AERA_F32) {
+        fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_tw), N / 2, N);
+        fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_t1k), 1024, 1024);
+        fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_twN), N, N);
+    } else {
+        fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_tw), N / 2, N);
+        fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_t1k), 1024, 1024);
+        fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_twN), N, N);
+    }
+    Plan *pl = new (std::nothrow) Plan();
+    if (!pl) return fail(AERA_ERR_ALLOC, "host allocation of a plan failed");
+    cudaError_t e = cudaMalloc(&pl->blob, total);
+    if (e != cudaSuccess) { delete pl; (void)cudaGetLastError(); return fail(AERA_ERR_ALLOC, "cudaMalloc(%zu) for a plan: %s", total, cudaGetErrorString(e)); }
+    e = cudaMemcpyAsync(pl->blob, h.data(), total, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s); // h goes out of scope
+    if (e != cudaSuccess) { cudaFree(pl->blob); delete pl; return cuda_fail(e, "plan upload"); }
+    unsigned char *b = static_cast<unsigned char *>(pl->blob);
+    pl->fs = fs;
+    pl->dev.N = N; pl->dev.logN = ilog2(N);
+    pl->dev.k_lo = k_lo; pl->dev.k_hi = k_hi; pl->dev.K = K;
+    pl->dev.bin_if = reinterpret_cast<const int *>(b + off_if);
+    pl->dev.bin_tf = reinterpret_cast<const double *>(b + off_tf);
+    pl->dev.tw = b + off_tw;
+    pl->dev.tw1024 = b + off_t1k;
+    pl->dev.twN = b + off_twN;
+    pat->plans[key] = pl;
+    *out = pl;
+    return AERA_OK;
+}
+
+TableGeom geom_of(const aera_pattern_desc_t &d)
+{
+    TableGeom g;
+    g.n_z = d.n_zenith; g.n_a = d.n_azimuth; g.n_f = d.n_freq; g.periodic = d.azimuth_periodic ? 1 : 0;
+    g.z0 = d.zenith0_deg; g.dz = d.dzenith_deg; g.a0 = d.azimuth0_deg; g.da = d.dazimuth_deg;
+    return g;
+}
+
+struct WsLayout {
+    size_t off_minv, off_scratch, off_spectra, total;
+};
+
+// Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
+WsLayout ws_layout(aera_op_t op, int dtype, int N, int K, long n_dirs, int n_stations)
+{
+    WsLayout w{};
+    const size_t cb = cplx_bytes(dtype);
+    size_t o = 0;
+    w.off_minv = o; o = align_up(o + (size_t)n_dirs * K * 4 * cb);
+    w.off_scratch = o; o = align_up(o + generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations));
+    w.off_spectra = o;
+    if (op == AERA_OP_SCAN) o = align_up(o + generic_scan_spectra_bytes(dtype, K, n_stations));
+    w.total = o > 0 ? o : kAlign;
+    return w;
+}
+
+aera_status_t check_common(const aera_pattern_t *pattern, int dtype, int n_stations, int n_samples, double fs_hz)
+{
+    if (!pattern) return fail(AERA_ERR_INVALID_ARG, "pattern is NULL");
+    if (dtype != AERA_F32 && dtype != AERA_F64) return fail(AERA_ERR_INVALID_ARG, "dtype=%d is neither AERA_F32 nor AERA_F64", dtype);
+    if (dtype != pattern->desc.dtype) return fail(AERA_ERR_DTYPE_MISMATCH, "dtype=%d but the pattern was uploaded as dtype=%d", dtype, pattern->desc.dtype);
+    if (n_stations <= 0) return fail(AERA_ERR_INVALID_ARG, "n_stations=%d must be positive", n_stations);
+    aera_status_t st = check_n(n_samples);
+    if (st != AERA_OK) return st;
+    if (!(fs_hz > 0) || !std::isfinite(fs_hz)) return fail(AERA_ERR_INVALID_ARG, "fs_hz must be positive and finite");
+    return AERA_OK;
+}
+
+bool misaligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
+
+} // namespace
+
+extern "C" {
+
+const char *aera_last_error(void) { return g_err; }
+const char *aera_version(void) { return "aera_unfold 0.1 (sm_100a)"; }
+unsigned long long aera_launch_count(void) { return g_launches.load(); }
+int aera_set_kernel_variant(int variant) { return g_variant.exchange(variant); }
+
+aera_status_t aera_pattern_upload(const aera_pattern_desc_t *desc, const void *H, int src_on_device,
+                                  void *cuda_stream, aera_pattern_t **out)
+{
+    if (!desc || !H || !out) return fail(AERA_ERR_INVALID_ARG, "desc, H and out must be non-NULL");
+    *out = nullptr;
+    if (desc->dtype != AERA_F32 && desc->dtype != AERA_F64) return fail(AERA_ERR_INVALID_ARG, "desc->dtype=%d invalid", desc->dtype);
+    if (desc->n_zenith < 2 || !(desc->dzenith_deg > 0)) return fail(AERA_ERR_INVALID_ARG, "zenith axis needs >= 2 nodes and a positive step");
+    if (desc->n_azimuth < (desc->azimuth_periodic ? 3 : 2) || !(desc->dazimuth_deg > 0))
+        return fail(AERA_ERR_INVALID_ARG, "azimuth axis needs >= %d nodes and a positive step", desc->azimuth_periodic ? 3 : 2);
+    if (desc->n_freq < 2 || desc->n_freq > 512 || !(desc->dfreq_hz > 0) || !(desc->freq0_hz > 0))
+        return fail(AERA_ERR_INVALID_ARG, "frequency axis needs 2..512 nodes, freq0 > 0 and a positive step");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    aera_pattern *p = new (std::nothrow) aera_pattern();
+    if (!p) return fail(AERA_ERR_ALLOC, "host allocation of a pattern handle failed");
+    p->desc = *desc;
+    const size_t n = (size_t)4 * desc->n_zenith * desc->n_azimuth * desc->n_freq;
+    p->table_bytes = n * cplx_bytes(desc->dtype);
+    void *d_src = nullptr;
+    cudaError_t e = cudaMalloc(&p->d_table, p->table_bytes);
+    if (e != cudaSuccess) { delete p; (void)cudaGetLastError(); return fail(AERA_ERR_ALLOC, "cudaMalloc(%zu) for the table: %s", n, cudaGetErrorString(e)); }
+    const void *src = H;
+    if (!src_on_device) {
+        e = cudaMalloc(&d_src, p->table_bytes);
+        if (e != cudaSuccess) { cudaFree(p->d_table); delete p; (void)cudaGetLastError(); return fail(AERA_ERR_ALLOC, "cudaMalloc staging: %s", cudaGetErrorString(e)); }
+        e = cudaMemcpyAsync(d_src, H, p->table_bytes, cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) { cudaFree(d_src); cudaFree(p->d_table); delete p; return cuda_fail(e, "table H2D copy"); }
+        src = d_src;
+    }
+    e = launch_repack(desc->dtype, src, p->d_table, desc->n_zenith, desc->n_azimuth, desc->n_freq, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (d_src) cudaFree(d_src);
+    if (e != cudaSuccess) { cudaFree(p->d_table); delete p; return cuda_fail(e, "table repack"); }
+    *out = p;
+    return AERA_OK;
+}
+
+aera_status_t aera_pattern_free(aera_pattern_t *p)
+{
+    if (!p) return AERA_OK;
+    for (auto &kv : p->plans) { cudaFree(kv.second->blob); delete kv.second; }
+    HostPipe &hp = p->pipe;
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(hp.d_in[i]); cudaFree(hp.d_out[i]); cudaFree(hp.d_amp[i]); cudaFree(hp.d_idx[i]);
+        cudaFree(hp.d_dirs[i]); cudaFree(hp.d_ws[i]);
+        if (hp.ev_in[i]) cudaEventDestroy(hp.ev_in[i]);
+        if (hp.ev_k[i]) cudaEventDestroy(hp.ev_k[i]);
+        if (hp.ev_out[i]) cudaEventDestroy(hp.ev_out[i]);
+    }
+    for (int i = 0; i < 3; ++i) if (hp.st[i]) cudaStreamDestroy(hp.st[i]);
+    cudaFree(p->d_table);
+    delete p;
+    return AERA_OK;
+}
+
+aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_hz, int *k_lo, int *k_hi)
+{
+    if (!pattern || !k_lo || !k_hi) return fail(AERA_ERR_INVALID_ARG, "pattern, k_lo and k_hi must be non-NULL");
+    aera_status_t st = check_n(n_samples);
+    if (st != AERA_OK) return st;
+    return compute_band(pattern->desc, n_samples, fs_hz, k_lo, k_hi);
+}
+
+size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,
+                            int n_stations, int n_samples, double fs_hz)
+{
+    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
+    if (check_common(pattern, dtype, n_stations, n_samples, fs_hz) != AERA_OK) return 0;
+    if (n_events_or_dirs < 0) { fail(AERA_ERR_INVALID_ARG, "negative count"); return 0; }
+    int k_lo, k_hi;
+    if (compute_band(pattern->desc, n_samples, fs_hz, &k_lo, &k_hi) != AERA_OK) return 0;
+    return ws_layout(op, dtype, n_samples, k_hi - k_lo + 1, n_events_or_dirs, n_stations).total;
+}
+
+aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                int n_samples, double fs_hz, const void *traces, const double *dirs,
+                                void *efield, void *peak_amp, int32_t *peak_idx,
+                                void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
+    if (st != AERA_OK) return st;
+    if (n_events < 0) return fail(AERA_ERR_INVALID_ARG, "n_events=%d is negative", n_events);
+    if (n_events == 0) return AERA_OK;
+    if (!traces || !dirs || !peak_amp || !peak_idx) return fail(AERA_ERR_INVALID_ARG, "traces, dirs, peak_amp and peak_idx must be non-NULL");
+    if (misaligned(traces, 16) || (efield && misaligned(efield, 16))) return fail(AERA_ERR_INVALID_ARG, "traces and efield must be 16-byte aligned");
+    if (misaligned(dirs, 8) || misaligned(peak_amp, real_bytes(dtype)) || misaligned(peak_idx, 4))
+        return fail(AERA_ERR_INVALID_ARG, "dirs / peak_amp / peak_idx are not aligned to their element size");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Plan *pl = nullptr;
+    st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
+    if (st != AERA_OK) return st;
+    const WsLayout w = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.K, n_events, n_stations);
+    if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
+        return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+
+    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv, s);
+    if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
+    e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
+                              ws + w.off_minv, ws + w.off_scratch, s);
+    if (e != cudaSuccess) return cuda_fail(e, "unfold kernel launch");
+    return AERA_OK;
+}
+
+aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int n_stations, int n_samples,
+                                   double fs_hz, const void *traces, long n_dirs, const double *dirs,
+                                   void *peak_amp, int32_t *peak_idx,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
+    if (st != AERA_OK) return st;
+    if (n_dirs < 0) return fail(AERA_ERR_INVALID_ARG, "n_dirs=%ld is negative", n_dirs);
+    if (n_dirs == 0) return AERA_OK;
+    if (n_dirs > 0x7fffffffL / 4) return fail(AERA_ERR_INVALID_ARG, "n_dirs=%ld too large", n_dirs);
+    if (!traces || !dirs || !peak_amp || !peak_idx) return fail(AERA_ERR_INVALID_ARG, "traces, dirs, peak_amp and peak_idx must be non-NULL");
+    if (misaligned(traces, 16)) return fail(AERA_ERR_INVALID_ARG, "traces must be 16-byte aligned");
+    if (misaligned(dirs, 8) || misaligned(peak_amp, real_bytes(dtype)) || misaligned(peak_idx, 4))
+        return fail(AERA_ERR_INVALID_ARG, "dirs / peak_amp / peak_idx are not aligned to their element size");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Plan *pl = nullptr;
+    st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
+    if (st != AERA_OK) return st;
+    const WsLayout w = ws_layout(AERA_OP_SCAN, dtype, n_samples, pl->dev.K, n_dirs, n_stations);
+    if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
+        return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+
+    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_dirs, ws + w.off_minv, s);
+    if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
+    e = launch_scan_generic(dtype, pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx,
+                            ws + w.off_spectra, ws + w.off_scratch, s);
+    if (e != cudaSuccess) return cuda_fail(e, "scan kernel launch");
+    return AERA_OK;
+}
+
+aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                     int n_samples, double fs_hz, const void *traces_host,
+                                     const double *dirs_host, void *efield_host, void *peak_amp_host,
+                                     int32_t *peak_idx_host)
+{
+    aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
+    if (st != AERA_OK) return st;
+    if (n_events < 0) return fail(AERA_ERR_INVALID_ARG, "n_events=%d is negative", n_events);
+    if (n_events == 0) return AERA_OK;
+    if (!traces_host || !dirs_host || !peak_amp_host || !peak_idx_host)
+        return fail(AERA_ERR_INVALID_ARG, "traces, dirs, peak_amp and peak_idx must be non-NULL");
+
+    const size_t rb = real_bytes(dtype);
+    const size_t unit_bytes = (size_t)2 * n_samples * rb;
+    const size_t event_bytes = unit_bytes * n_stations;
+    // chunk: ~64 MB of traces per stage, at least one event
+    long chunk_events = (long)((size_t)(64u << 20) / event_bytes);
+    if (chunk_events < 1) chunk_events = 1;
+    if (chunk_events > n_events) chunk_events = n_events;
+
+    HostPipe &hp = pattern->pipe;
+    cudaError_t e;
+    if (!hp.ready) {
+        for (int i = 0; i < 3; ++i) { e = cudaStreamCreateWithFlags(&hp.st[i], cudaStreamNonBlocking); if (e != cudaSuccess) return cuda_fail(e, "stream create"); }
+        for (int i = 0; i < 2; ++i) {
+            if ((e = cudaEventCreateWithFlags(&hp.ev_in[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "event create");
+            if ((e = cudaEventCreateWithFlags(&hp.ev_k[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "event create");
+            if ((e = cudaEventCreateWithFlags(&hp.ev_out[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "event create");
+        }
+        hp.ready = true;
+    }
+    Plan *pl = nullptr;
+    st = get_plan(pattern, n_samples, fs_hz, hp.st[1], &pl);
+    if (st != AERA_OK) return st;
+    const size_t need_trace = (size_t)chunk_events * event_bytes;
+    const size_t need_units = (size_t)chunk_events * n_stations;
+    const size_t need_ws = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.K, chunk_events, n_stations).total;
+    if (need_trace > hp.cap_trace_bytes || need_units > hp.cap_units || need_ws > hp.cap_ws || (size_t)chunk_events > hp.cap_events) {
+        cudaDeviceSynchronize();
+        for (int i = 0; i < 2; ++i) {
+            cudaFree(hp.d_in[i]); cudaFree(hp.d_out[i]); cudaFree(hp.d_amp[i]); cudaFree(hp.d_idx[i]); cudaFree(hp.d_dirs[i]); cudaFree(hp.d_ws[i]);
+            hp.d_in[i] = hp.d_out[i] = hp.d_amp[i] = hp.d_ws[i] = nullptr; hp.d_idx[i] = nullptr; hp.d_dirs[i] = nullptr;
+            bool ok = cudaMalloc(&hp.d_in[i], need_trace) == cudaSuccess && cudaMalloc(&hp.d_out[i], need_trace) == cudaSuccess &&
+                      cudaMalloc(&hp.d_amp[i], need_units * 8) == cudaSuccess && cudaMalloc((void **)&hp.d_idx[i], need_units * 4) == cudaSuccess &&
+                      cudaMalloc((void **)&hp.d_dirs[i], (size_t)chunk_events * 16) == cudaSuccess && cudaMalloc(&hp.d_ws[i], need_ws) == cudaSuccess;
+            if (!ok) { (void)cudaGetLastError(); hp.cap_trace_bytes = hp.cap_units = hp.cap_ws = hp.cap_events = 0; return fail(AERA_ERR_ALLOC, "cudaMalloc of host-pipeline staging buffers failed"); }
+        }
+        hp.cap_trace_bytes = need_trace; hp.cap_units = need_units; hp.cap_ws = need_ws; hp.cap_events = (size_t)chunk_events;
+    }
+
+    const unsigned char *tin = static_cast<const unsigned char *>(traces_host);
+    unsigned char *eout = static_cast<unsigned char *>(efield_host);
+    unsigned char *aout = static_cast<unsigned char *>(peak_amp_host);
+    long done = 0; int it = 0;
+    while (done < n_events) {
+        const int b = it & 1;
+        const long ne = (n_events - done < chunk_events) ? (n_events - done) : chunk_events;
+        const size_t units = (size_t)ne * n_stations;
+        // stage b's input buffer is free once the kernel that read it (2 iterations ago) finished;
+        // its output buffers are free once their D2H copy finished.
+        if (it >= 2) {
+            if ((e = cudaStreamWaitEvent(hp.st[0], hp.ev_k[b], 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
+            if ((e = cudaStreamWaitEvent(hp.st[1], hp.ev_out[b], 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
+        }
+        if ((e = cudaMemcpyAsync(hp.d_in[b], tin + (size_t)done * event_bytes, (size_t)ne * event_bytes, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return cuda_fail(e, "H2D traces");
+        if ((e = cudaMemcpyAsync(hp.d_dirs[b], dirs_host + 2 * done, (size_t)ne * 16, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return cuda_fail(e, "H2D dirs");
+        cudaEventRecord(hp.ev_in[b], hp.st[0]);
+        cudaStreamWaitEvent(hp.st[1], hp.ev_in[b], 0);
+        st = aera_unfold_batch(pattern, dtype, (int)ne, n_stations, n_samples, fs_hz, hp.d_in[b], hp.d_dirs[b],
+                               efield_host ? hp.d_out[b] : nullptr, hp.d_amp[b], hp.d_idx[b], hp.d_ws[b], hp.cap_ws, hp.st[1]);
+        if (st != AERA_OK) { cudaDeviceSynchronize(); return st; }
+        cudaEventRecord(hp.ev_k[b], hp.st[1]);
+        cudaStreamWaitEvent(hp.st[2], hp.ev_k[b], 0);
+        if (efield_host)
+            if ((e = cudaMemcpyAsync(eout + (size_t)done * event_bytes, hp.d_out[b], (size_t)ne * event_bytes, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H efield");
+        if ((e = cudaMemcpyAsync(aout + (size_t)done * n_stations * rb, hp.d_amp[b], units * rb, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H amp");
+        if ((e = cudaMemcpyAsync(peak_idx_host + (size_t)done * n_stations, hp.d_idx[b], units * 4, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H idx");
+        cudaEventRecord(hp.ev_out[b], hp.st[2]);
+        done += ne; ++it;
+    }
+    for (int i = 0; i < 3; ++i)
+        if ((e = cudaStreamSynchronize(hp.st[i])) != cudaSuccess) return cuda_fail(e, "host pipeline synchronise");
+    return AERA_OK;
+}
+
+} // extern "C"

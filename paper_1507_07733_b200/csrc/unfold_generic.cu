@@ -1,0 +1,314 @@
+// Generic unfolding kernels: any power-of-two N in [64, 65536], fp32 or fp64.
+//
+// This is the library's reference-quality CUDA path: one CTA per station, in-place radix-2
+// transforms on three complex buffers (forward spectrum, Z_theta, Z_phi) that live in shared
+// memory when they fit (3*N*sizeof(complex) <= 192 KB) and otherwise in a per-CTA slice of the
+// caller's workspace (L2-resident).  It covers every size the specialised warp kernels
+// (unfold_w32.cu) do not, and tests run it against them.  Steps per station:
+//   a1 load v0 + i v1 (bit-reversed)           a2 forward FFT (two real transforms for one)
+//   a4 E = Minv V on the in-band bins           a5 two inverse FFTs of the one-sided spectra
+//   a6 e_p = Re z_p, env^2 = |z_theta|^2+|z_phi|^2, max / lowest argmax
+// (a3, the pattern evaluation, is pattern.cu's minv_kernel, once per event.)
+#include "aera_internal.h"
+
+namespace aera {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr size_t kSmemBudget = 192 * 1024;
+
+template <typename T>
+__device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b)
+{
+    cx<T> r;
+    r.re = a.re * b.re - a.im * b.im;
+    r.im = a.re * b.im + a.im * b.re;
+    return r;
+}
+
+// In-place radix-2 decimation-in-time FFT of `nbuf` buffers of N points whose inputs are already
+// in bit-reversed order. tw[m] = exp(-2 pi i m / N), m < N/2; inverse uses the conjugate.
+template <typename T, bool INVERSE, int NBUF>
+__device__ void cta_fft(cx<T> *b0, cx<T> *b1, int N, int logN, const cx<T> *__restrict__ tw)
+{
+    for (int s = 0; s < logN; ++s) {
+        const int half = 1 << s;
+        const int tstride = (N >> 1) >> s;
+        for (int j = threadIdx.x; j < (N >> 1); j += blockDim.x) {
+            const int pos = j & (half - 1);
+            const int i0 = ((j - pos) << 1) + pos;
+            const int i1 = i0 + half;
+            cx<T> w = tw[pos * tstride];
+            if (INVERSE) w.im = -w.im;
+            {
+                cx<T> a = b0[i0], t = cmul(w, b0[i1]);
+                b0[i0].re = a.re + t.re; b0[i0].im = a.im + t.im;
+                b0[i1].re = a.re - t.re; b0[i1].im = a.im - t.im;
+            }
+            if (NBUF == 2) {
+                cx<T> a = b1[i0], t = cmul(w, b1[i1]);
+                b1[i0].re = a.re + t.re; b1[i0].im = a.im + t.im;
+                b1[i1].re = a.re - t.re; b1[i1].im = a.im - t.im;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// (value, index) max with lowest index on ties; every reduction stage uses the same rule.
+template <typename T>
+__device__ __forceinline__ void argmax_combine(T &v, int &i, T ov, int oi)
+{
+    if (ov > v || (ov == v && oi < i)) { v = ov; i = oi; }
+}
+
+template <typename T>
+__device__ void cta_argmax(T v, int i, T *amp_out, int32_t *idx_out)
+{
+    __shared__ T sv[32];
+    __shared__ int si[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        T ov = __shfl_xor_sync(0xffffffffu, v, o);
+        int oi = __shfl_xor_sync(0xffffffffu, i, o);
+        argmax_combine(v, i, ov, oi);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sv[warp] = v; si[warp] = i; }
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = blockDim.x >> 5;
+        v = lane < nw ? sv[lane] : (T)-1;
+        i = lane < nw ? si[lane] : 0x7fffffff;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            T ov = __shfl_xor_sync(0xffffffffu, v, o);
+            int oi = __shfl_xor_sync(0xffffffffu, i, o);
+            argmax_combine(v, i, ov, oi);
+        }
+        if (lane == 0) { *amp_out = sqrt(v); *idx_out = i; }
+    }
+    __syncthreads();
+}
+
+template <typename T>
+__device__ __forceinline__ void zero_buffers(cx<T> *B, cx<T> *C, int N)
+{
+    for (int n = threadIdx.x; n < N; n += blockDim.x) {
+        B[n].re = 0; B[n].im = 0; C[n].re = 0; C[n].im = 0;
+    }
+}
+
+// a5 + a6 on buffers B (theta) and C (phi) holding the bit-reversed one-sided spectra.
+template <typename T>
+__device__ void inverse_and_peak(cx<T> *B, cx<T> *C, const PlanDev &p, T *ef, T *amp, int32_t *idx)
+{
+    const int N = p.N;
+    cta_fft<T, true, 2>(B, C, N, p.logN, (const cx<T> *)p.tw);
+    T best = (T)-1; int bi = 0x7fffffff;
+    for (int n = threadIdx.x; n < N; n += blockDim.x) {
+        cx<T> zt = B[n], zp = C[n];
+        if (ef) { ef[n] = zt.re; ef[N + n] = zp.re; }
+        T e2 = zt.re * zt.re + zt.im * zt.im + zp.re * zp.re + zp.im * zp.im;
+        argmax_combine(best, bi, e2, n);
+    }
+    cta_argmax<T>(best, bi, amp, idx);
+}
+
+template <typename T>
+__device__ void forward_spectrum(cx<T> *A, const PlanDev &p, const T *v)
+{
+    const int N = p.N, sh = 32 - p.logN;
+    for (int n = threadIdx.x; n < N; n += blockDim.x) {
+        const int r = (int)(__brev((unsigned)n) >> sh);
+        A[r].re = v[n]; A[r].im = v[N + n];
+    }
+    __syncthreads();
+    cta_fft<T, false, 1>(A, nullptr, N, p.logN, (const cx<T> *)p.tw);
+}
+
+// C[k] = V0[k] + i V1[k], conj C[N-k] = V0[k] - i V1[k]  (v0, v1 real)
+template <typename T>
+__device__ __forceinline__ void split_channels(cx<T> c, cx<T> m, cx<T> &v0, cx<T> &v1)
+{
+    v0.re = (T)0.5 * (c.re + m.re); v0.im = (T)0.5 * (c.im - m.im);
+    v1.re = (T)0.5 * (c.im + m.im); v1.im = (T)-0.5 * (c.re - m.re);
+}
+
+template <typename T>
+__device__ __forceinline__ void apply_minv(const cx<T> *__restrict__ M, cx<T> v0, cx<T> v1, cx<T> &et, cx<T> &ep)
+{
+    cx<T> a = cmul(M[0], v0), b = cmul(M[1], v1);
+    et.re = a.re + b.re; et.im = a.im + b.im;
+    a = cmul(M[2], v0); b = cmul(M[3], v1);
+    ep.re = a.re + b.re; ep.im = a.im + b.im;
+}
+
+template <typename T, bool SMEM>
+__global__ void __launch_bounds__(kThreads)
+unfold_generic_kernel(PlanDev p, long n_units, int n_stations, const T *__restrict__ traces, T *efield,
+                      T *__restrict__ amp, int32_t *__restrict__ idx, const cx<T> *__restrict__ minv,
+                      cx<T> *scratch)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = p.N, sh = 32 - p.logN;
+    cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * 3 * N;
+    cx<T> *B = A + N, *C = B + N;
+
+    for (long u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const long ev = u / n_stations;
+        zero_buffers(B, C, N);
+        forward_spectrum<T>(A, p, traces + (size_t)u * 2 * N); // ends with __syncthreads
+        const cx<T> *M = minv + (size_t)ev * p.K * 4;
+        for (int j = threadIdx.x; j < p.K; j += blockDim.x) {
+            const int k = p.k_lo + j;
+            cx<T> v0, v1, et, ep;
+            split_channels(A[k], A[N - k], v0, v1);
+            apply_minv(M + 4 * j, v0, v1, et, ep);
+            const int r = (int)(__brev((unsigned)k) >> sh);
+            B[r] = et; C[r] = ep;
+        }
+        __syncthreads();
+        inverse_and_peak<T>(B, C, p, efield ? efield + (size_t)u * 2 * N : nullptr, amp + u, idx + u);
+    }
+}
+
+// Scan, kernel A: forward transform once per station, in-band spectra to the workspace [S][2][K].
+template <typename T, bool SMEM>
+__global__ void __launch_bounds__(kThreads)
+scan_forward_generic_kernel(PlanDev p, int n_stations, const T *__restrict__ traces, cx<T> *__restrict__ spectra,
+                            cx<T> *scratch)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = p.N;
+    cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * 3 * N;
+    for (int s = blockIdx.x; s < n_stations; s += gridDim.x) {
+        forward_spectrum<T>(A, p, traces + (size_t)s * 2 * N);
+        for (int j = threadIdx.x; j < p.K; j += blockDim.x) {
+            const int k = p.k_lo + j;
+            cx<T> v0, v1;
+            split_channels(A[k], A[N - k], v0, v1);
+            spectra[((size_t)s * 2 + 0) * p.K + j] = v0;
+            spectra[((size_t)s * 2 + 1) * p.K + j] = v1;
+        }
+        __syncthreads();
+    }
+}
+
+// Scan, kernel B: one CTA per (direction, station) pair.
+template <typename T, bool SMEM>
+__global__ void __launch_bounds__(kThreads)
+scan_inverse_generic_kernel(PlanDev p, int n_stations, long n_pairs, const cx<T> *__restrict__ spectra,
+                            const cx<T> *__restrict__ minv, T *__restrict__ amp, int32_t *__restrict__ idx,
+                            cx<T> *scratch)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = p.N, sh = 32 - p.logN;
+    cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * 3 * N;
+    cx<T> *B = A + N, *C = B + N;
+    for (long pr = blockIdx.x; pr < n_pairs; pr += gridDim.x) {
+        const long d = pr / n_stations;
+        const int s = (int)(pr % n_stations);
+        zero_buffers(B, C, N);
+        __syncthreads();
+        const cx<T> *M = minv + (size_t)d * p.K * 4;
+        for (int j = threadIdx.x; j < p.K; j += blockDim.x) {
+            cx<T> et, ep;
+            apply_minv(M + 4 * j, spectra[((size_t)s * 2 + 0) * p.K + j], spectra[((size_t)s * 2 + 1) * p.K + j], et, ep);
+            const int r = (int)(__brev((unsigned)(p.k_lo + j)) >> sh);
+            B[r] = et; C[r] = ep;
+        }
+        __syncthreads();
+        inverse_and_peak<T>(B, C, p, (T *)nullptr, amp + pr, idx + pr);
+    }
+}
+
+size_t elem_bytes(int dtype) { return dtype == AERA_F32 ? sizeof(cx<float>) : sizeof(cx<double>); }
+bool fits_smem(int dtype, int N) { return (size_t)3 * N * elem_bytes(dtype) <= kSmemBudget; }
+long generic_grid(long n_units) { return n_units < 148L * 4 ? n_units : 148L * 4; }
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t bytes)
+{
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <typename T>
+cudaError_t launch_unfold_t(int dtype, const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield,
+                            void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
+{
+    const long grid = generic_grid(n_units);
+    if (fits_smem(dtype, p.N)) {
+        size_t smem = (size_t)3 * p.N * sizeof(cx<T>);
+        cudaError_t e = set_smem(unfold_generic_kernel<T, true>, smem);
+        if (e != cudaSuccess) return e;
+        unfold_generic_kernel<T, true><<<(unsigned)grid, kThreads, smem, s>>>(
+            p, n_units, n_stations, (const T *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, nullptr);
+    } else {
+        unfold_generic_kernel<T, false><<<(unsigned)grid, kThreads, 0, s>>>(
+            p, n_units, n_stations, (const T *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, (cx<T> *)scratch);
+    }
+    count_launches(1);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_scan_t(int dtype, const PlanDev &p, int n_stations, const void *traces, long n_dirs, const void *minv,
+                          void *amp, int32_t *idx, void *spectra, void *scratch, cudaStream_t s)
+{
+    const long n_pairs = n_dirs * (long)n_stations;
+    const long gridA = generic_grid(n_stations), gridB = generic_grid(n_pairs);
+    if (fits_smem(dtype, p.N)) {
+        size_t smem = (size_t)3 * p.N * sizeof(cx<T>);
+        cudaError_t e = set_smem(scan_forward_generic_kernel<T, true>, smem);
+        if (e != cudaSuccess) return e;
+        e = set_smem(scan_inverse_generic_kernel<T, true>, smem);
+        if (e != cudaSuccess) return e;
+        scan_forward_generic_kernel<T, true><<<(unsigned)gridA, kThreads, smem, s>>>(
+            p, n_stations, (const T *)traces, (cx<T> *)spectra, nullptr);
+        scan_inverse_generic_kernel<T, true><<<(unsigned)gridB, kThreads, smem, s>>>(
+            p, n_stations, n_pairs, (const cx<T> *)spectra, (const cx<T> *)minv, (T *)amp, idx, nullptr);
+    } else {
+        scan_forward_generic_kernel<T, false><<<(unsigned)gridA, kThreads, 0, s>>>(
+            p, n_stations, (const T *)traces, (cx<T> *)spectra, (cx<T> *)scratch);
+        scan_inverse_generic_kernel<T, false><<<(unsigned)gridB, kThreads, 0, s>>>(
+            p, n_stations, n_pairs, (const cx<T> *)spectra, (const cx<T> *)minv, (T *)amp, idx, (cx<T> *)scratch);
+    }
+    count_launches(2);
+    return cudaGetLastError();
+}
+
+} // namespace
+
+size_t generic_scratch_bytes(int dtype, int N, long n_units)
+{
+    if (fits_smem(dtype, N)) return 0;
+    return (size_t)generic_grid(n_units) * 3 * N * elem_bytes(dtype);
+}
+
+size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations)
+{
+    return (size_t)n_stations * 2 * K * elem_bytes(dtype);
+}
+
+cudaError_t launch_unfold_generic(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces,
+                                  void *efield, void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
+{
+    const long n_units = n_events * (long)n_stations;
+    if (n_units <= 0) return cudaSuccess;
+    return dtype == AERA_F32
+               ? launch_unfold_t<float>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s)
+               : launch_unfold_t<double>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s);
+}
+
+cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, const void *traces, long n_dirs,
+                                const void *minv, void *amp, int32_t *idx, void *spectra, void *scratch, cudaStream_t s)
+{
+    if (n_dirs <= 0 || n_stations <= 0) return cudaSuccess;
+    return dtype == AERA_F32
+               ? launch_scan_t<float>(dtype, p, n_stations, traces, n_dirs, minv, amp, idx, spectra, scratch, s)
+               : launch_scan_t<double>(dtype, p, n_stations, traces, n_dirs, minv, amp, idx, spectra, scratch, s);
+}
+
+} // namespace aera

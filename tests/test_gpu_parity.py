@@ -1,0 +1,221 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle on identical seeded
+inputs. Run on the B200 box: python -m pytest tests -m gpu -x -q
+"""
+import numpy as np
+import pytest
+import torch
+
+import aera_inputs as ai
+
+pytestmark = pytest.mark.gpu
+
+from parity import TOL, compare, compare_peaks  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def B():
+    import paper_1507_07733_b200.binding as b
+    assert torch.cuda.is_available()
+    return b
+
+
+@pytest.fixture(scope="module")
+def orc():
+    import oracle
+    return oracle
+
+
+_tables = {}
+
+
+def table_for(wl):
+    key = (wl.grid, wl.dtype)
+    if key not in _tables:
+        _tables[key] = ai.pattern_table(wl.grid, wl.complex_dtype)
+    return _tables[key]
+
+
+def run_gpu_batch(B, wl, H, traces, dirs, variant=0, inplace=False, want_efield=True):
+    dt = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    old = B.aera_set_kernel_variant(variant)
+    try:
+        tr = torch.from_numpy(traces).cuda()
+        dd = torch.from_numpy(dirs).cuda()
+        ef, amp, idx = B.aera_unfold_batch(pat, tr, dd, wl.fs_hz, efield=tr if inplace else None, want_efield=want_efield)
+        torch.cuda.synchronize()
+        out = (ef.cpu().numpy() if ef is not None else None, amp.cpu().numpy(), idx.cpu().numpy())
+    finally:
+        B.aera_set_kernel_variant(old)
+        pat.free()
+    return out
+
+
+def oracle_batch(orc, wl, H, traces, dirs):
+    E, S = traces.shape[:2]
+    return orc.unfold_batch(wl.grid, H, wl.fs_hz, traces.reshape(E * S, 2, -1), np.repeat(dirs, S, axis=0), want_env2=True)
+
+
+def check(wl, gpu, ref):
+    ef, amp, idx = gpu
+    U = len(ref["amp"])
+    rep = compare(wl.dtype, ef.reshape(U, 2, -1) if ef is not None else None, amp.ravel(), idx.ravel(), ref)
+    print(f"\n[parity cfg{wl.config}] {rep}")
+    assert rep.ok(TOL[wl.dtype]), str(rep)
+    return rep
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config0_all_units(B, orc, variant):
+    wl = ai.WORKLOADS[0]
+    H = table_for(wl)
+    tr, dirs, _, _ = ai.make_batch(wl, [0])
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, variant), oracle_batch(orc, wl, H, tr, dirs))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_subsample(B, orc, variant):
+    wl = ai.WORKLOADS[1]
+    H = table_for(wl)
+    events = [0, 1, 17, 999]
+    tr, dirs, _, _ = ai.make_batch(wl, events)
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, variant), oracle_batch(orc, wl, H, tr, dirs))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config3_fp64_subsample(B, orc, variant):
+    wl = ai.WORKLOADS[3]
+    H = table_for(wl)
+    events = [0, 1, 2, 3, 5000, 9999, 42]
+    tr, dirs, _, _ = ai.make_batch(wl, events)
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, variant), oracle_batch(orc, wl, H, tr, dirs))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config4_long_trace_subsample(B, orc, variant):
+    wl = ai.WORKLOADS[4]
+    H = table_for(wl)
+    n_st = 8 if variant == 0 else 4
+    tr, dirs, _, _ = ai.make_batch(wl, [0], n_stations=n_st)
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, variant), oracle_batch(orc, wl, H, tr, dirs))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config2_scan(B, orc, variant):
+    wl = ai.WORKLOADS[2]
+    H = table_for(wl)
+    ev = ai.make_event(wl, 0)
+    alld = ai.scan_directions()
+    rng = np.random.default_rng(2)
+    pick = set(rng.choice(len(alld), size=58, replace=False).tolist())
+    # the four grid corners, phi = 358 (periodic wrap) and a theta = 80 row
+    pick |= {0, 179, len(alld) - 180, len(alld) - 1, 20 * 180 + 179, 40 * 180 + 90}
+    dirs = alld[sorted(pick)]
+    assert len(dirs) >= 64
+    dt = B.AERA_F32
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    old = B.aera_set_kernel_variant(variant)
+    try:
+        amp, idx = B.aera_scan_directions(pat, torch.from_numpy(ev.traces).cuda(), torch.from_numpy(dirs).cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+    finally:
+        B.aera_set_kernel_variant(old)
+        pat.free()
+    oamp, oidx = orc.scan(wl.grid, H, wl.fs_hz, ev.traces, dirs)
+    rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx)
+    print(f"\n[parity cfg2 scan] {rep}")
+    assert rep.max_amp <= TOL["f32"]["amp"] and rep.idx_miss == 0, str(rep)
+
+
+# ------------------------------------------------------------------ sizes and edge cases
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("N", [64, 128, 256, 512, 1024, 2048, 4096, 8192])
+def test_all_sizes_small_batch(B, orc, N, dtype):
+    """Every supported power of two up to 8192 (16384-65536 are covered by config 4), ragged batch:
+    3 events x 5 stations; fs chosen so the band keeps ~N/4 bins."""
+    base = ai.WORKLOADS[0]
+    wl = ai.Workload(90, "sizes", 3, 5, N, 200e6, dtype, base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    tr, dirs, _, _ = ai.make_batch(wl, range(3))
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs), oracle_batch(orc, wl, H, tr, dirs))
+
+
+def test_directions_wrap_clamp_and_nodes(B, orc):
+    wl = ai.WORKLOADS[0]
+    H = table_for(wl)
+    tr, _, _, _ = ai.make_batch(wl, range(8))
+    dirs = np.array([[35.0, 125.0],      # exactly a grid node
+                     [12.3, 359.9],      # last azimuth cell, wraps to node 0
+                     [12.3, -10.0],      # negative azimuth
+                     [45.0, 725.0],      # two periods up
+                     [0.0, 0.0],         # table corner
+                     [60.0, 360.0],      # phi == period
+                     [89.0, 200.0],      # near the singular theta = 90 nodes (still regular)
+                     [-5.0, 10.0]])      # clamped zenith
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs), oracle_batch(orc, wl, H, tr, dirs))
+
+
+def test_inplace_and_peaks_only(B, orc):
+    wl = ai.WORKLOADS[1]
+    H = table_for(wl)
+    tr, dirs, _, _ = ai.make_batch(wl, [3], n_stations=9)
+    ref = oracle_batch(orc, wl, H, tr, dirs)
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, inplace=True), ref)
+    ef, amp, idx = run_gpu_batch(B, wl, H, tr, dirs, want_efield=False)
+    assert ef is None
+    check(wl, (None, amp, idx), ref)
+
+
+def test_zero_events_and_errors(B):
+    wl = ai.WORKLOADS[0]
+    H = table_for(wl)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        tr = torch.zeros((0, 7, 2, 256), device="cuda")
+        dd = torch.zeros((0, 2), dtype=torch.float64, device="cuda")
+        ef, amp, idx = B.aera_unfold_batch(pat, tr, dd, wl.fs_hz)
+        assert amp.numel() == 0
+        tr = torch.zeros((1, 7, 2, 256), device="cuda")
+        dd = torch.zeros((1, 2), dtype=torch.float64, device="cuda")
+        with pytest.raises(B.AeraError) as e:
+            B.aera_unfold_batch(pat, torch.zeros((1, 7, 2, 200), device="cuda"), dd, wl.fs_hz, workspace=B.alloc_workspace(1 << 20))
+        assert e.value.status == 2
+        with pytest.raises(B.AeraError) as e:
+            B.aera_unfold_batch(pat, tr.double(), dd, wl.fs_hz, workspace=B.alloc_workspace(1 << 20))
+        assert e.value.status == 3
+        with pytest.raises(B.AeraError) as e:
+            B.aera_unfold_batch(pat, tr, dd, wl.fs_hz, workspace=B.alloc_workspace(256))
+        assert e.value.status == 4
+        with pytest.raises(B.AeraError) as e:  # band reaches Nyquist: fs = 150 MHz < 2 * 80 MHz
+            B.aera_unfold_batch(pat, tr, dd, 150e6, workspace=B.alloc_workspace(1 << 20))
+        assert e.value.status == 7
+        with pytest.raises(B.AeraError) as e:  # misaligned traces
+            B.aera_unfold_batch(pat, torch.zeros(1 * 7 * 2 * 256 + 1, device="cuda")[1:].view(1, 7, 2, 256), dd, wl.fs_hz)
+        assert e.value.status == 1
+        assert B.aera_band(pat, 256, 200e6) == (39, 102)
+    finally:
+        pat.free()
+
+
+def test_host_pipeline_matches_device_path(B):
+    wl = ai.WORKLOADS[1]
+    H = table_for(wl)
+    tr, dirs, _, _ = ai.make_batch(wl, range(6), n_stations=31)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        t_h = torch.from_numpy(tr).pin_memory(); d_h = torch.from_numpy(dirs).pin_memory()
+        ef_h, amp_h, idx_h = B.aera_unfold_batch_host(pat, t_h, d_h, wl.fs_hz)
+        ef_d, amp_d, idx_d = B.aera_unfold_batch(pat, t_h.cuda(), d_h.cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        assert torch.equal(ef_h, ef_d.cpu()) and torch.equal(amp_h, amp_d.cpu()) and torch.equal(idx_h, idx_d.cpu())
+    finally:
+        pat.free()
+
+
+def test_library_is_loaded_and_counts_launches(B):
+    n0 = B.aera_launch_count()
+    wl = ai.WORKLOADS[0]
+    tr, dirs, _, _ = ai.make_batch(wl, [0])
+    run_gpu_batch(B, wl, table_for(wl), tr, dirs)
+    assert B.aera_launch_count() >= n0 + 3  # repack + minv + unfold
+    assert B.LIBRARY_PATH.endswith("libaera_unfold.so")
