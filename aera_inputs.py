@@ -222,3 +222,32 @@ def make_batch(wl: Workload, events, n_stations: int | None = None):
     amp = np.stack([e.amplitude for e in evs])
     arr = np.stack([e.arrival for e in evs])
     return traces, dirs, amp, arr
+
+
+def _event_worker(args):
+    cfg, ev, n_st = args
+    e = make_event(WORKLOADS[cfg], ev, n_st)
+    return e.traces, e.direction_deg, e.amplitude, e.arrival
+
+
+def make_batch_parallel(wl: Workload, events, n_stations: int | None = None, workers: int | None = None,
+                        out_traces=None):
+    """make_batch with a process pool (input synthesis only). `out_traces` may be a preallocated
+    [E][S][2][N] array (e.g. a view of pinned memory) that receives the traces."""
+    import concurrent.futures as cf
+    import os
+
+    events = [int(e) for e in events]
+    S = wl.n_stations if n_stations is None else n_stations
+    if out_traces is None:
+        out_traces = np.empty((len(events), S, 2, wl.n_samples), dtype=wl.real_dtype)
+    dirs = np.empty((len(events), 2)); amp = np.empty((len(events), S)); arr = np.empty((len(events), S))
+    workers = workers or min(32, os.cpu_count() or 1)
+    if workers <= 1 or len(events) < 4:
+        for i, e in enumerate(events):
+            out_traces[i], dirs[i], amp[i], arr[i] = _event_worker((wl.config, e, n_stations))
+        return out_traces, dirs, amp, arr
+    with cf.ProcessPoolExecutor(max_workers=workers) as ex:
+        for i, r in enumerate(ex.map(_event_worker, [(wl.config, e, n_stations) for e in events], chunksize=8)):
+            out_traces[i], dirs[i], amp[i], arr[i] = r
+    return out_traces, dirs, amp, arr

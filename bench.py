@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native E-field unfolding path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1|3|4]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One "step" = one pass of the whole hot path (pattern evaluation + 2x2 inverse per event, then the
+fused FFT / solve / inverse FFT / envelope / argmax kernel) over one batch of synthetic input.
+Default workload: BASELINE.json configs[1] (1000 events x 124 stations x 2 channels x 2048 fp32).
+Metric: station-traces unfolded per second (whole job, all ranks). Prints ONE JSON line on rank 0.
+
+`--impl reference`: there is no reference implementation of this paper (it ships no code); per the
+task contract that arm times the CPU oracle (oracle/, plain C, naive O(N K) DFT sums) on the host
+cores, on a bounded sample of the same workload per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import aera_inputs as ai  # noqa: E402
+
+METRIC = "station-traces unfolded/sec (2ch x 2048 fp32) and % of B200 HBM peak"
+UNIT = "station-traces/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_ read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s earlier measurement on this pool)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows = []
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def algorithmic_bytes_per_unit(wl) -> int:
+    """one read + one write of the 2 x N traces + peak (amp + int32 idx)."""
+    b = 4 if wl.dtype == "f32" else 8
+    return 2 * wl.n_samples * b * 2 + b + 4
+
+
+def build_inputs(wl, n_events, rank, pinned: bool):
+    """Canonical seeded events [rank*n_events, ...) of the workload, generated on the host."""
+    import torch
+    shape = (n_events, wl.n_stations, 2, wl.n_samples)
+    tdt = torch.float32 if wl.dtype == "f32" else torch.float64
+    host = torch.empty(shape, dtype=tdt, pin_memory=pinned)
+    # canonical block: up to 200 distinct events, tiled (distinct addresses >> L2)
+    n_canon = min(n_events, 200)
+    _, dirs_c, amp_c, arr_c = ai.make_batch_parallel(wl, range(rank * n_canon, (rank + 1) * n_canon),
+                                                     out_traces=host[:n_canon].numpy())
+    reps = -(-n_events // n_canon)
+    for r in range(1, reps):
+        lo = r * n_canon; hi = min(n_events, lo + n_canon)
+        host[lo:hi] = host[: hi - lo]
+    dirs = np.tile(dirs_c, (reps, 1))[:n_events]
+    amp = np.tile(amp_c, (reps, 1))[:n_events]
+    arr = np.tile(arr_c, (reps, 1))[:n_events]
+    return host, torch.from_numpy(np.ascontiguousarray(dirs)), amp, arr
+
+
+def run_reference(args, wl):
+    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    cores = oracle.num_threads()
+    ev_per_step = max(1, min(wl.n_events, (cores * 2 * 124) // wl.n_stations // 4)) if wl.n_samples <= 4096 else 1
+    n_st = wl.n_stations if wl.n_samples <= 4096 else min(wl.n_stations, cores)
+    tr, dirs, _, _ = ai.make_batch(wl, range(ev_per_step), n_stations=n_st)
+    U = tr.shape[0] * tr.shape[1]
+    trf = tr.reshape(U, 2, -1); dd = np.repeat(dirs, tr.shape[1], axis=0)
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle.unfold_batch(wl.grid, H, wl.fs_hz, trf, dd)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.unfold_batch(wl.grid, H, wl.fs_hz, trf, dd)
+    dt = time.perf_counter() - t0
+    val = U * args.steps / dt
+    sample = f"{ev_per_step} event(s) x {n_st} stations of config {wl.config} per step ({U} units), OpenMP over units"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, aera_inputs.py)",
+        "config": {"workload": f"BASELINE configs[{wl.config}] {wl.name}: bounded sample per step", "n_samples": wl.n_samples,
+                   "n_stations": n_st, "events_per_step": ev_per_step},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[1, 3, 4])
+    ap.add_argument("--events", type=int, default=0, help="override the number of events (0 = the config's)")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 auto, 1 generic)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    wl = ai.WORKLOADS[args.config]
+
+    if args.impl == "reference":
+        run_reference(args, wl)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (no CPU fallback exists)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    import paper_1507_07733_b200.binding as B
+    B.aera_set_kernel_variant(args.variant)
+
+    n_events = args.events or wl.n_events
+    if args.config == 3 and not args.events:
+        n_events = 2000  # 26 GB in + 26 GB out at the full 10000 events; 2000 events (10.5 GB) keeps setup short; >> L2
+    dt_code = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt_code), H)
+
+    t_setup = time.time()
+    host_tr, host_dirs, amp_inj, arr_inj = build_inputs(wl, n_events, rank, pinned=True)
+    host_dirs = host_dirs.pin_memory()
+    d_tr = host_tr.cuda(non_blocking=True); d_dirs = host_dirs.cuda(non_blocking=True)
+    d_ef = torch.empty_like(d_tr)
+    d_amp = torch.empty((n_events, wl.n_stations), dtype=d_tr.dtype, device="cuda")
+    d_idx = torch.empty((n_events, wl.n_stations), dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_UNFOLD, pat, dt_code, n_events, wl.n_stations, wl.n_samples, wl.fs_hz))
+    torch.cuda.synchronize()
+    t_setup = time.time() - t_setup
+    n_units = n_events * wl.n_stations
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.aera_unfold_batch(pat, d_tr, d_dirs, wl.fs_hz, efield=d_ef, peak_amp=d_amp, peak_idx=d_idx, workspace=ws, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, barrier + sync both sides
+    sampler = ClockSampler(local_rank); sampler.start()
+    B.aera_profile_enable(True)
+    l0 = B.aera_launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = B.aera_launch_count() - l0
+    B.aera_profile_enable(False)
+    k_ms, k_n = B.aera_profile_read(B.KERNEL_IDS["unfold"])
+    m_ms, m_n = B.aera_profile_read(B.KERNEL_IDS["minv"])
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms_total], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n_units / (ms_step * 1e-3)
+
+    # ---- plausibility of the timed outputs (cheap property check at full size; parity is in tests/)
+    amp_h = d_amp.cpu().numpy(); idx_h = d_idx.cpu().numpy()
+    strong = amp_inj > 300.0
+    ok_idx = float(np.mean(np.abs(idx_h[strong] - arr_inj[strong]) <= 3))
+    sane = bool(np.isfinite(amp_h).all() and ok_idx > 0.98)
+
+    # ---- roofline of the dominant kernel (batched unfold), live CUDA-event timing inside the library
+    peak, peak_src = load_peaks()
+    bytes_unit = algorithmic_bytes_per_unit(wl)
+    k_avg_ms = k_ms / max(k_n, 1)
+    achieved = n_units * bytes_unit / (k_avg_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "kernel": "unfold (fused FFT+solve+iFFT+envelope)", "kernel_ms": k_avg_ms, "kernel_share_of_step": k_avg_ms / ms_step,
+                "minv_kernel_ms": m_ms / max(m_n, 1), "algorithmic_bytes_per_unit": bytes_unit, "peak_source": peak_src,
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+    tpath = os.path.join(ROOT, "profiles", f"traffic_config{wl.config}.json")
+    if os.path.exists(tpath):
+        try:
+            roofline["traffic"] = json.load(open(tpath)).get("dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        out_ef = torch.empty(host_tr.shape, dtype=host_tr.dtype, pin_memory=True)
+        out_amp = torch.empty((n_events, wl.n_stations), dtype=host_tr.dtype, pin_memory=True)
+        out_idx = torch.empty((n_events, wl.n_stations), dtype=torch.int32, pin_memory=True)
+        n_e2e = max(2, min(args.steps, 5))
+        B.aera_unfold_batch_host(pat, host_tr, host_dirs, wl.fs_hz, efield=out_ef, peak_amp=out_amp, peak_idx=out_idx)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            B.aera_unfold_batch_host(pat, host_tr, host_dirs, wl.fs_hz, efield=out_ef, peak_amp=out_amp, peak_idx=out_idx)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([t_e2e], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); t_e2e = float(t.item())
+        same = bool(torch.equal(out_idx, d_idx.cpu()))
+        e2e = {"value": world * n_units / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(host_tr.numel() * host_tr.element_size() + host_dirs.numel() * 8),
+               "d2h_bytes_per_step": int(out_ef.numel() * out_ef.element_size() + out_amp.numel() * out_amp.element_size() + out_idx.numel() * 4),
+               "ms_per_step": t_e2e * 1e3, "steps": n_e2e, "api": "aera_unfold_batch_host (pinned host buffers, 3-stream chunk pipeline)",
+               "matches_device_path": same}
+        del out_ef
+
+    # ---- CPU oracle baseline on the box's host cores (rank 0, N=1 only), bounded sample
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        cores = oracle.num_threads()
+        n_ev_s = {1: 32, 3: 16, 4: 1}[wl.config]
+        n_st_s = wl.n_stations if wl.config != 4 else min(wl.n_stations, cores)
+        tr_s = host_tr[:n_ev_s, :n_st_s].numpy(); U = n_ev_s * n_st_s
+        dd = np.repeat(host_dirs[:n_ev_s].numpy(), n_st_s, axis=0)
+        t0 = time.perf_counter()
+        r = oracle.unfold_batch(wl.grid, H, wl.fs_hz, tr_s.reshape(U, 2, -1), dd, want_efield=False)
+        dt = time.perf_counter() - t0
+        agree = float(np.mean(r["idx"] == idx_h[:n_ev_s, :n_st_s].ravel()))
+        cpu = {"value": U / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {n_ev_s} events x {n_st_s} stations of the timed batch ({U} units, {dt:.1f} s wall), OpenMP over units",
+               "peak_idx_agreement_with_gpu": agree}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": wl.dtype, "data": "synthetic (seeded, aera_inputs.py; stands in for AERA traces and antenna patterns)",
+            "config": {"workload": f"BASELINE configs[{wl.config}] {wl.name}: {n_events} events x {wl.n_stations} stations x 2 ch x {wl.n_samples} {wl.dtype} per GPU",
+                       "n_events": n_events, "n_stations": wl.n_stations, "n_samples": wl.n_samples, "fs_hz": wl.fs_hz,
+                       "l2_policy": f"inputs+outputs {2 * d_tr.numel() * d_tr.element_size() / 1e9:.1f} GB per step >> 126 MB L2 (no flush needed)",
+                       "kernel_variant": "auto" if args.variant == 0 else "generic", "sharding": "events across ranks, no collective"},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "outputs_sane": sane, "strong_pulse_idx_within_3": ok_idx, "setup_s": round(t_setup, 1), "library": B.aera_version(),
+        }
+        print(json.dumps(line), flush=True)
+    pat.free()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -153,6 +153,15 @@ int aera_set_kernel_variant(int variant);
 /* Number of kernel launches this library has enqueued since load (monotonic, all threads). */
 unsigned long long aera_launch_count(void);
 
+/* Per-kernel device timing with CUDA events recorded on the stream each kernel is launched on
+ * (used by bench.py for the roofline figures; off by default, costs two event records per launch).
+ * aera_profile_enable(1) clears earlier records and starts recording; (0) stops. Returns the
+ * previous state. aera_profile_read waits for the recorded events of one kernel and returns the
+ * summed duration and the number of launches. kernel_id: 0 table repack, 1 pattern
+ * evaluation + 2x2 inverse (per event/direction), 2 batched unfold, 3 scan forward, 4 scan inverse. */
+int aera_profile_enable(int on);
+aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches);
+
 /* Message for the most recent non-OK status on this thread ("" if none). Static storage. */
 const char *aera_last_error(void);
 

@@ -21,7 +21,7 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
            "aera_scan_directions", "aera_unfold_batch_host", "aera_set_kernel_variant", "aera_launch_count",
-           "aera_last_error", "aera_version")
+           "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read")
 
 
 class AeraError(RuntimeError):
@@ -70,6 +70,10 @@ def _load():
     lib.aera_set_kernel_variant.argtypes = [C.c_int]
     lib.aera_set_kernel_variant.restype = C.c_int
     lib.aera_launch_count.restype = C.c_ulonglong
+    lib.aera_profile_enable.argtypes = [C.c_int]
+    lib.aera_profile_enable.restype = C.c_int
+    lib.aera_profile_read.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
+    lib.aera_profile_read.restype = C.c_int
     lib.aera_last_error.restype = C.c_char_p
     lib.aera_version.restype = C.c_char_p
     return lib, path
@@ -137,6 +141,20 @@ def aera_launch_count() -> int:
 
 def aera_set_kernel_variant(variant: int) -> int:
     return int(_lib.aera_set_kernel_variant(int(variant)))
+
+
+KERNEL_IDS = {"repack": 0, "minv": 1, "unfold": 2, "scan_fwd": 3, "scan_inv": 4}
+
+
+def aera_profile_enable(on: bool) -> int:
+    return int(_lib.aera_profile_enable(1 if on else 0))
+
+
+def aera_profile_read(kernel_id: int):
+    """-> (total_ms, launches) of one kernel since aera_profile_enable(True)."""
+    ms, n = C.c_double(), C.c_long()
+    _check(_lib.aera_profile_read(kernel_id, C.byref(ms), C.byref(n)))
+    return ms.value, n.value
 
 
 def aera_pattern_upload(desc: PatternDesc, H, stream=None) -> Pattern:

@@ -32,6 +32,16 @@ struct PlanDev {
 void count_launches(unsigned n);
 int kernel_variant();
 
+// Optional per-kernel CUDA-event timing (aera_profile_enable / aera_profile_read in the C ABI).
+enum KernelId { KID_REPACK = 0, KID_MINV = 1, KID_UNFOLD = 2, KID_SCAN_FWD = 3, KID_SCAN_INV = 4, KID_COUNT = 5 };
+void prof_begin(int kid, cudaStream_t s); // no-ops unless profiling is enabled
+void prof_end(int kid, cudaStream_t s);
+struct ProfScope {
+    int kid; cudaStream_t s;
+    ProfScope(int k, cudaStream_t st) : kid(k), s(st) { prof_begin(kid, s); }
+    ~ProfScope() { prof_end(kid, s); }
+};
+
 // ---- pattern.cu
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);
 // Minv[d][j][4] = (2/N) * H(theta_d, phi_d, f_{k_lo+j})^-1, rows (theta0, theta1, phi0, phi1).

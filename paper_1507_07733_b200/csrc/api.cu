@@ -22,6 +22,38 @@ int kernel_variant() { return g_variant.load(std::memory_order_relaxed); }
 
 static thread_local char g_err[512] = "";
 
+// ---- per-kernel event timing -------------------------------------------------------------
+struct ProfRec { int kid; cudaEvent_t e0, e1; };
+static std::mutex g_prof_mu;
+static std::atomic<int> g_prof_on{0};
+static std::vector<ProfRec> g_prof_recs;
+static std::vector<cudaEvent_t> g_prof_pool;
+static thread_local cudaEvent_t g_prof_open = nullptr;
+
+static cudaEvent_t prof_get_event()
+{
+    if (!g_prof_pool.empty()) { cudaEvent_t e = g_prof_pool.back(); g_prof_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+void prof_begin(int, cudaStream_t s)
+{
+    if (!g_prof_on.load(std::memory_order_relaxed)) return;
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_open = prof_get_event();
+    cudaEventRecord(g_prof_open, s);
+}
+void prof_end(int kid, cudaStream_t s)
+{
+    if (!g_prof_on.load(std::memory_order_relaxed) || !g_prof_open) return;
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    cudaEvent_t e1 = prof_get_event();
+    cudaEventRecord(e1, s);
+    g_prof_recs.push_back({kid, g_prof_open, e1});
+    g_prof_open = nullptr;
+}
+
 static aera_status_t fail(aera_status_t st, const char *fmt, ...)
 {
     va_list ap;
@@ -232,6 +264,35 @@ bool misaligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p
 } // namespace
 
 extern "C" {
+
+int aera_profile_enable(int on)
+{
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    int prev = g_prof_on.exchange(on ? 1 : 0);
+    if (on) {
+        for (auto &r : g_prof_recs) { g_prof_pool.push_back(r.e0); g_prof_pool.push_back(r.e1); }
+        g_prof_recs.clear();
+    }
+    return prev;
+}
+
+aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches)
+{
+    if (!total_ms || !launches) return fail(AERA_ERR_INVALID_ARG, "total_ms and launches must be non-NULL");
+    if (kernel_id < 0 || kernel_id >= KID_COUNT) return fail(AERA_ERR_INVALID_ARG, "kernel_id %d out of range", kernel_id);
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    double sum = 0; long n = 0;
+    for (auto &r : g_prof_recs) {
+        if (r.kid != kernel_id) continue;
+        cudaError_t e = cudaEventSynchronize(r.e1);
+        float ms = 0;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.e0, r.e1);
+        if (e != cudaSuccess) return cuda_fail(e, "profile event read");
+        sum += ms; ++n;
+    }
+    *total_ms = sum; *launches = n;
+    return AERA_OK;
+}
 
 const char *aera_last_error(void) { return g_err; }
 const char *aera_version(void) { return "aera_unfold 0.1 (sm_100a)"; }

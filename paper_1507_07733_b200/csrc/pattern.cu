@@ -31,6 +31,7 @@ __global__ void repack_kernel(const cx<T> *__restrict__ src, cx<T> *__restrict__
 
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s)
 {
+    ProfScope prof(KID_REPACK, s);
     size_t total = (size_t)n_z * n_a * n_f * 4;
     int blocks = (int)((total + 255) / 256);
     if (blocks > 148 * 16) blocks = 148 * 16;
@@ -190,6 +191,7 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
                         const double *dirs, long n_dirs, void *minv, cudaStream_t s)
 {
     if (n_dirs <= 0) return cudaSuccess;
+    ProfScope prof(KID_MINV, s);
     size_t smem = minv_smem_bytes(dtype, g.n_f);
     double scale = 2.0 / (double)p.N;
     cudaError_t e;

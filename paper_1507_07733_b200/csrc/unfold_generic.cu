@@ -238,6 +238,7 @@ template <typename T>
 cudaError_t launch_unfold_t(int dtype, const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield,
                             void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
 {
+    ProfScope prof(KID_UNFOLD, s);
     const long grid = generic_grid(n_units);
     if (fits_smem(dtype, p.N)) {
         size_t smem = (size_t)3 * p.N * sizeof(cx<T>);
@@ -265,13 +266,21 @@ cudaError_t launch_scan_t(int dtype, const PlanDev &p, int n_stations, const voi
         if (e != cudaSuccess) return e;
         e = set_smem(scan_inverse_generic_kernel<T, true>, smem);
         if (e != cudaSuccess) return e;
-        scan_forward_generic_kernel<T, true><<<(unsigned)gridA, kThreads, smem, s>>>(
-            p, n_stations, (const T *)traces, (cx<T> *)spectra, nullptr);
+        {
+            ProfScope prof(KID_SCAN_FWD, s);
+            scan_forward_generic_kernel<T, true><<<(unsigned)gridA, kThreads, smem, s>>>(
+                p, n_stations, (const T *)traces, (cx<T> *)spectra, nullptr);
+        }
+        ProfScope prof(KID_SCAN_INV, s);
         scan_inverse_generic_kernel<T, true><<<(unsigned)gridB, kThreads, smem, s>>>(
             p, n_stations, n_pairs, (const cx<T> *)spectra, (const cx<T> *)minv, (T *)amp, idx, nullptr);
     } else {
-        scan_forward_generic_kernel<T, false><<<(unsigned)gridA, kThreads, 0, s>>>(
-            p, n_stations, (const T *)traces, (cx<T> *)spectra, (cx<T> *)scratch);
+        {
+            ProfScope prof(KID_SCAN_FWD, s);
+            scan_forward_generic_kernel<T, false><<<(unsigned)gridA, kThreads, 0, s>>>(
+                p, n_stations, (const T *)traces, (cx<T> *)spectra, (cx<T> *)scratch);
+        }
+        ProfScope prof(KID_SCAN_INV, s);
         scan_inverse_generic_kernel<T, false><<<(unsigned)gridB, kThreads, 0, s>>>(
             p, n_stations, n_pairs, (const cx<T> *)spectra, (const cx<T> *)minv, (T *)amp, idx, (cx<T> *)scratch);
     }
