@@ -44,9 +44,12 @@ struct ProfScope {
 
 // ---- pattern.cu
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);
-// Minv[d][j][4] = (2/N) * H(theta_d, phi_d, f_{k_lo+j})^-1, rows (theta0, theta1, phi0, phi1).
+// Minv[d][j][4] = scale * H(theta_d, phi_d, f_{k_lo+j})^-1.
+//   MINV_ROWS   : complex entries (theta<-V0, theta<-V1, phi<-V0, phi<-V1)            (generic kernels)
+//   MINV_PACKED : reals {t0.re, p0.re, t0.im, p0.im, t1.re, p1.re, t1.im, p1.im}       (warp kernels)
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1 };
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
-                        const double *dirs, long n_dirs, void *minv, cudaStream_t s);
+                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s);
 size_t minv_smem_bytes(int dtype, int n_f);
 
 // ---- unfold_generic.cu
@@ -58,5 +61,10 @@ size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations);
 cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, const void *traces,
                                 long n_dirs, const void *minv, void *amp, int32_t *idx,
                                 void *spectra, void *scratch, cudaStream_t s);
+
+// ---- unfold_w32.cu: warp-per-station kernel for N = 2048 fp32 with the band below N/2
+bool w32_supported(int dtype, const PlanDev &p);
+cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s);
 
 } // namespace aera

@@ -394,10 +394,16 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
 
-    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv, s);
+    const bool warp_path = kernel_variant() == 0 && w32_supported(dtype, pl->dev);
+    // the warp kernel forms 2 V_c, so its matrix carries 1/N instead of 2/N
+    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
+                                warp_path ? MINV_PACKED : MINV_ROWS, (warp_path ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
-    e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
-                              ws + w.off_minv, ws + w.off_scratch, s);
+    if (warp_path)
+        e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
+    else
+        e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
+                                  ws + w.off_minv, ws + w.off_scratch, s);
     if (e != cudaSuccess) return cuda_fail(e, "unfold kernel launch");
     return AERA_OK;
 }
@@ -425,7 +431,8 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
 
-    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_dirs, ws + w.off_minv, s);
+    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_dirs, ws + w.off_minv,
+                                MINV_ROWS, 2.0 / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     e = launch_scan_generic(dtype, pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx,
                             ws + w.off_spectra, ws + w.off_scratch, s);

@@ -121,7 +121,7 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restrict__ dirs,
             const int *__restrict__ bin_if, const double *__restrict__ bin_tf, int K, double scale,
-            cx<T> *__restrict__ minv)
+            int layout, cx<T> *__restrict__ minv)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
@@ -174,10 +174,17 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         if (den != 0.0) { ir = scale * dr / den; ii = -scale * di / den; }
         cx<T> *o = minv + ((size_t)d * K + j) * 4;
         // E_theta = ( h3 V0 - h1 V1)/det ; E_phi = (-h2 V0 + h0 V1)/det
-        o[0].re = (T)(hr[3] * ir - hi[3] * ii);  o[0].im = (T)(hr[3] * ii + hi[3] * ir);
-        o[1].re = (T)(-(hr[1] * ir - hi[1] * ii)); o[1].im = (T)(-(hr[1] * ii + hi[1] * ir));
-        o[2].re = (T)(-(hr[2] * ir - hi[2] * ii)); o[2].im = (T)(-(hr[2] * ii + hi[2] * ir));
-        o[3].re = (T)(hr[0] * ir - hi[0] * ii);  o[3].im = (T)(hr[0] * ii + hi[0] * ir);
+        cx<T> mt0, mt1, mp0, mp1; // theta <- V0, theta <- V1, phi <- V0, phi <- V1
+        mt0.re = (T)(hr[3] * ir - hi[3] * ii);    mt0.im = (T)(hr[3] * ii + hi[3] * ir);
+        mt1.re = (T)(-(hr[1] * ir - hi[1] * ii)); mt1.im = (T)(-(hr[1] * ii + hi[1] * ir));
+        mp0.re = (T)(-(hr[2] * ir - hi[2] * ii)); mp0.im = (T)(-(hr[2] * ii + hi[2] * ir));
+        mp1.re = (T)(hr[0] * ir - hi[0] * ii);    mp1.im = (T)(hr[0] * ii + hi[0] * ir);
+        if (layout == MINV_ROWS) {
+            o[0] = mt0; o[1] = mt1; o[2] = mp0; o[3] = mp1;
+        } else { // MINV_PACKED: (theta, phi) side by side so a packed f32x2 / double2 load yields both
+            o[0].re = mt0.re; o[0].im = mp0.re; o[1].re = mt0.im; o[1].im = mp0.im;
+            o[2].re = mt1.re; o[2].im = mp1.re; o[3].re = mt1.im; o[3].im = mp1.im;
+        }
     }
 }
 
@@ -188,23 +195,22 @@ size_t minv_smem_bytes(int dtype, int n_f)
 }
 
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
-                        const double *dirs, long n_dirs, void *minv, cudaStream_t s)
+                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s)
 {
     if (n_dirs <= 0) return cudaSuccess;
     ProfScope prof(KID_MINV, s);
     size_t smem = minv_smem_bytes(dtype, g.n_f);
-    double scale = 2.0 / (double)p.N;
     cudaError_t e;
     if (dtype == AERA_F32) {
         e = cudaFuncSetAttribute(minv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                             p.K, scale, (cx<float> *)minv);
+                                                             p.K, scale, layout, (cx<float> *)minv);
     } else {
         e = cudaFuncSetAttribute(minv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                              p.K, scale, (cx<double> *)minv);
+                                                              p.K, scale, layout, (cx<double> *)minv);
     }
     count_launches(1);
     return cudaGetLastError();
