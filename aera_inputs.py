@@ -18,7 +18,7 @@ Using the analytic response for the synthesis (instead of interpolating the
 perturbed table) keeps the method's interpolation out of this module; the
 consequence is that an unfolded pulse differs from the injected one by the
 table's ~5 % perturbation, like a real antenna-model uncertainty would
-(reading R3).
+(reading R16).
 
 Everything is a pure function of (config id, event index) through
 `numpy.random.default_rng([7733, config, event])`, so any event can be

@@ -25,7 +25,7 @@
  * Readings of the paper where it is silent or garbled are listed in DESIGN.md
  * (section "Readings"); the ones that matter here: envelope = modulus of the analytic
  * signal (R1), forward kernel e^{-2 pi i nk/N} unnormalised, inverse 1/N (R5),
- * DC and Nyquist bins always zero (R4), band edges inclusive (R3'),
+ * DC and Nyquist bins always zero (R4), band edges inclusive (R3),
  * det == 0 -> bin zeroed (R8), zenith clamped / azimuth wrapped (R12, R7).
  *
  * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
