@@ -46,7 +46,8 @@ struct ProfScope {
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);
 // Minv[d][j][4] = scale * H(theta_d, phi_d, f_{k_lo+j})^-1.
 //   MINV_ROWS   : complex entries (theta<-V0, theta<-V1, phi<-V0, phi<-V1)            (generic kernels)
-//   MINV_PACKED : reals {t0.re, p0.re, t0.im, p0.im, t1.re, p1.re, t1.im, p1.im}       (warp kernels)
+//   MINV_PACKED : per direction two planes A[K], B[K] of 4 reals: A = {t0.re, p0.re, t0.im, p0.im},
+//                 B = {t1.re, p1.re, t1.im, p1.im}                                     (warp kernels)
 enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1 };
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
                         const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s);

@@ -13,6 +13,7 @@
 // used: its 8-bit fractional weights explain the paper's +-0.8 % discrepancy (L75) and cannot meet
 // the 1e-4 parity bound.
 #include "aera_internal.h"
+#include "async_copy.cuh"
 
 namespace aera {
 
@@ -41,36 +42,6 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
         repack_kernel<double><<<blocks, 256, 0, s>>>((const cx<double> *)src, (cx<double> *)dst, n_z, n_a, n_f);
     count_launches(1);
     return cudaGetLastError();
-}
-
-// ---------------------------------------------------------------- mbarrier / TMA bulk helpers
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t done = 0;
-    while (!done) {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    }
 }
 
 struct DirCell {
@@ -181,9 +152,11 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         mp1.re = (T)(hr[0] * ir - hi[0] * ii);    mp1.im = (T)(hr[0] * ii + hi[0] * ir);
         if (layout == MINV_ROWS) {
             o[0] = mt0; o[1] = mt1; o[2] = mp0; o[3] = mp1;
-        } else { // MINV_PACKED: (theta, phi) side by side so a packed f32x2 / double2 load yields both
-            o[0].re = mt0.re; o[0].im = mp0.re; o[1].re = mt0.im; o[1].im = mp0.im;
-            o[2].re = mt1.re; o[2].im = mp1.re; o[3].re = mt1.im; o[3].im = mp1.im;
+        } else { // MINV_PACKED: two planes per direction, (theta, phi) side by side so a packed
+                 // f32x2 load yields both: A[j] = {t0.re, p0.re, t0.im, p0.im}, B[j] = {t1.re, p1.re, t1.im, p1.im}
+            cx<T> *a = minv + (size_t)d * K * 4 + (size_t)j * 2, *b = a + (size_t)K * 2;
+            a[0].re = mt0.re; a[0].im = mp0.re; a[1].re = mt0.im; a[1].im = mp0.im;
+            b[0].re = mt1.re; b[0].im = mp1.re; b[1].re = mt1.im; b[1].im = mp1.im;
         }
     }
 }
