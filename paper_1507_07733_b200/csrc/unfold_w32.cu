@@ -25,7 +25,7 @@
 // (shared-memory counter) issues the copy of event e+2 into the slot it vacates.
 //
 // HBM traffic per station: 16 KB read once (L2-prefetched one station ahead with
-// cp.async.bulk.prefetch.L2), 16 KB + 8 B written once. Shared memory per warp: one 8.25 KB padded
+// cp.async.bulk.prefetch.L2), 16 KB + 8 B written once (two 8 KB TMA bulk stores from shared memory). Shared memory per warp: one 8.25 KB padded
 // transpose buffer + a stash for the in-band spectrum (needed twice, s = 0 and 1).
 //
 // The in-band rows (bins k = lane + 32 row) are template parameters, so every per-row decision is
@@ -139,19 +139,22 @@ __device__ __forceinline__ void emit_even(const R (&zr)[32], const R (&zi)[32], 
     });
 }
 
+// Odd pass: lane l, row b reads its parked (theta, phi) even sample, and writes the (even, odd)
+// pair of phi back to the same 8 bytes of `park` and the pair of theta to the same offset of
+// `out_theta`: both buffers end up holding 8 KB of finished output in global-memory order, which
+// two TMA bulk stores then write (no LSU store traffic, every sector written once and in full).
 template <bool HAS_EF>
-__device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], int lane, const R *park, float *ef,
+__device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], int lane, R *park, R *out_theta,
                                          float &best, int &bb)
 {
     static_for<0, 32>([&](auto bc) {
         constexpr int b = decltype(bc)::value;
         if (HAS_EF) {
-            float ot, op;
+            float ot, op, et, ep;
             L::unpack(zr[b], ot, op);
-            const float2 ev = *reinterpret_cast<const float2 *>(park + b * 32 + lane); // (theta, phi) at n = 2m
-            const int m = lane + 32 * b;
-            *reinterpret_cast<float2 *>(ef + 2 * m) = make_float2(ev.x, ot);
-            *reinterpret_cast<float2 *>(ef + 2 * kM + 2 * m) = make_float2(ev.y, op);
+            L::unpack(park[b * 32 + lane], et, ep);
+            out_theta[b * 32 + lane] = L::pack(et, ot);
+            park[b * 32 + lane] = L::pack(ep, op);
         }
         R q = L::mul(zr[b], zr[b]);
         q = L::fma(zi[b], zi[b], q);
@@ -248,7 +251,15 @@ unfold_w32_kernel(W32Params p)
             });
 
             // ---- a2: forward FFT of g_0, g_1
-            fft1024(A, B, X, T, lane);
+            fft32<L>(A, B);
+            pass_twiddle(A, B, T, lane);
+            if (HAS_EF) { // the previous station's bulk stores must have read X / X2 before they are reused
+                if (lane == 0) bulk_wait_group_read0();
+                __syncwarp();
+            }
+            transpose_plane(A, X, lane);
+            transpose_plane(B, X, lane);
+            fft32<L>(A, B);
 
             // ---- mirror exchange: publish the rows that are somebody's bin 1024-k
             static_for<G::kMirLo, G::kMirHi + 1>([&](auto rc) {
@@ -327,8 +338,16 @@ unfold_w32_kernel(W32Params p)
             });
             __syncwarp(); // stash consumed by every lane before its region becomes the transpose buffer
             fft1024(Zi, Zr, X2, T, lane);   // X holds the parked even samples
-            emit_odd<HAS_EF>(Zr, Zi, lane, X, ef, best1, b1);
-            __syncwarp(); // parked samples read before the next station's transposes reuse X
+            emit_odd<HAS_EF>(Zr, Zi, lane, X, X2, best1, b1);
+            if (HAS_EF) {
+                fence_proxy_async_smem(); // this lane's shared-memory writes -> visible to the TMA engine
+                __syncwarp();
+                if (lane == 0) {
+                    tma_bulk_s2g(ef, X2, kM * 8);           // e_theta[0..2048)
+                    tma_bulk_s2g(ef + 2 * kM, X, kM * 8);   // e_phi[0..2048)
+                    bulk_commit_group();
+                }
+            }
 
             // ---- a6: lane result (lowest index on ties), then warp argmax with the same rule
             float best = best0; int bi = 2 * (lane + 32 * b0);
@@ -365,6 +384,7 @@ unfold_w32_kernel(W32Params p)
             }
         }
     }
+    if (HAS_EF && lane == 0) bulk_wait_group0(); // shared memory must outlive the last bulk stores
 }
 
 template <int K2LO, int K2HI, bool MINV_SMEM>
