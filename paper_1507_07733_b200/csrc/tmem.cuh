@@ -1,0 +1,67 @@
+// Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) used as a lane-private scratchpad.
+//
+// No tensor-core instruction is issued anywhere in this library (the path is not a contraction);
+// what the warp kernels need is a second place, besides shared memory, to park data that a lane
+// writes and later reads back ITSELF: the in-band spectrum between the two inverse transforms and
+// the even output samples until their odd neighbours exist. With the .32x32b shape of
+// tcgen05.ld/st, thread t of warp w owns TMEM lane 32 (w % 4) + t and reads/writes consecutive
+// 32-bit columns of it: no bank conflicts by construction, a datapath separate from the LSU /
+// shared-memory crossbar (measured on B200, 8 warps/SM: STTM.x2 1.05, LDTM.x2 1.5 cycles per
+// 256-byte warp access against 2.0 for LDS.64/STS.64, and the two overlap), and it frees 17.5 KB of
+// shared memory per warp. SASS: UTCALLOC / STTM / LDTM.
+#pragma once
+#include <cstdint>
+
+namespace aera {
+
+// One warp allocates all 512 columns (the kernels run one CTA per SM) and publishes the base
+// address through shared memory; the caller follows with tmem_publish_sync().
+__device__ __forceinline__ void tmem_alloc_all(uint32_t *base_in_smem)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;"
+                 ::"r"((uint32_t)__cvta_generic_to_shared(base_in_smem)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_free_all(uint32_t base)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
+
+// Address of column `col` in the lane quarter that warp `warp` may access.
+__device__ __forceinline__ uint32_t tmem_addr(uint32_t base, int warp, int col)
+{
+    return base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)col;
+}
+
+// 64 bits per thread (two consecutive columns). The address must be warp-uniform.
+__device__ __forceinline__ void tmem_st64(uint32_t addr, unsigned long long v)
+{
+    asm volatile("{\n.reg .b32 lo, hi;\nmov.b64 {lo, hi}, %1;\n"
+                 "tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {lo, hi};\n}" ::"r"(addr), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long tmem_ld64(uint32_t addr)
+{
+    unsigned long long v;
+    asm volatile("{\n.reg .b32 lo, hi;\n"
+                 "tcgen05.ld.sync.aligned.32x32b.x2.b32 {lo, hi}, [%1];\nmov.b64 %0, {lo, hi};\n}" : "=l"(v) : "r"(addr) : "memory");
+    return v;
+}
+// Results of earlier tmem_ld64 calls may be used only after this. The loaded values are passed
+// through as in/out operands so the compiler cannot schedule a consumer above the wait.
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void tmem_wait_ld(unsigned long long (&v)[N])
+{
+    static_assert(N == 4 || N == 8, "chunk sizes used by the kernels");
+    if constexpr (N == 8)
+        asm volatile("tcgen05.wait::ld.sync.aligned;"
+                     : "+l"(v[0]), "+l"(v[1]), "+l"(v[2]), "+l"(v[3]), "+l"(v[4]), "+l"(v[5]), "+l"(v[6]), "+l"(v[7]) :: "memory");
+    else
+        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(v[0]), "+l"(v[1]), "+l"(v[2]), "+l"(v[3]) :: "memory");
+}
+// Earlier tmem_st64 calls of this thread are complete (visible to its later tmem_ld64).
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+} // namespace aera

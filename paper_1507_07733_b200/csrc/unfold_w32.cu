@@ -25,14 +25,21 @@
 // (shared-memory counter) issues the copy of event e+2 into the slot it vacates.
 //
 // HBM traffic per station: 16 KB read once (L2-prefetched one station ahead with
-// cp.async.bulk.prefetch.L2), 16 KB + 8 B written once (two 8 KB TMA bulk stores from shared memory). Shared memory per warp: one 8.25 KB padded
-// transpose buffer + a stash for the in-band spectrum (needed twice, s = 0 and 1).
+// cp.async.bulk.prefetch.L2), 16 KB + 8 B written once, as (even, odd) sample pairs: 8 bytes per
+// lane, 256 contiguous bytes per store instruction, every 32-byte sector written once and in full.
+//
+// Lane-private scratch lives in tensor memory (tmem.cuh), not in shared memory: the in-band
+// spectrum E (needed twice, s = 0 and 1) and Re z of the even samples (until the odd pass can pair
+// them up). That leaves one 10 KB transpose / mirror-exchange buffer per warp in shared memory, so
+// twelve warps (168 registers each) fit on an SM instead of eight: three warps per scheduler hide
+// each other's shared-memory and global-memory latencies.
 //
 // The in-band rows (bins k = lane + 32 row) are template parameters, so every per-row decision is
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
 #include "aera_internal.h"
 #include "async_copy.cuh"
 #include "fft32.cuh"
+#include "tmem.cuh"
 
 namespace aera {
 namespace {
@@ -41,10 +48,9 @@ using L = LaneF32x2;
 using R = F2;
 
 constexpr int kM = 1024;
-constexpr int kWarps = 8;
 constexpr int kXBytes = 33 * 32 * 8;   // padded 32x32 transpose buffer, 8-byte elements
 constexpr int kTabBytes = 2 * 1024 * 8; // T + TS
-constexpr int kCtlBytes = 128;          // mbarriers + counters
+constexpr int kCtlBytes = 128;          // mbarriers + counters + TMEM base address
 
 struct W32Params {
     const float *traces;
@@ -114,6 +120,11 @@ __device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const floa
     fft32<L>(A, B);
 }
 
+__device__ __forceinline__ void st_global_b64(void *p, R v)
+{
+    asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
+}
+
 // Outputs of one inverse transform: lane a, register b holds z[m = a + 32 b] of (theta, phi);
 // sample index n = 2 m + parity. Both routines track the maximum of env^2 over b (ascending,
 // strict >, so the lowest b wins ties).
@@ -121,15 +132,14 @@ __device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const floa
 // Even samples come out one whole inverse transform before the odd ones. Writing them straight to
 // global memory would fill only half of every 32-byte sector, and the half-written sectors get
 // evicted from L2 (ECC read-modify-write in DRAM: +35 % read, +13 % write traffic measured). So
-// the even pass parks Re z in shared memory and the odd pass stores (even, odd) pairs: 8 bytes per
-// lane, 256 contiguous bytes per instruction, every sector written once and in full.
+// the even pass parks Re z (theta, phi) in this lane's tensor-memory columns and the odd pass
+// stores (even, odd) pairs.
 template <bool HAS_EF>
-__device__ __forceinline__ void emit_even(const R (&zr)[32], const R (&zi)[32], int lane, R *park,
-                                          float &best, int &bb)
+__device__ __forceinline__ void emit_even(const R (&zr)[32], const R (&zi)[32], uint32_t tpark, float &best, int &bb)
 {
     static_for<0, 32>([&](auto bc) {
         constexpr int b = decltype(bc)::value;
-        if (HAS_EF) park[b * 32 + lane] = zr[b];
+        if (HAS_EF) tmem_st64(tpark + 2 * b, zr[b].v);
         R q = L::mul(zr[b], zr[b]);
         q = L::fma(zi[b], zi[b], q);
         float qt, qp;
@@ -139,33 +149,45 @@ __device__ __forceinline__ void emit_even(const R (&zr)[32], const R (&zi)[32], 
     });
 }
 
-// Odd pass: lane l, row b reads its parked (theta, phi) even sample, and writes the (even, odd)
-// pair of phi back to the same 8 bytes of `park` and the pair of theta to the same offset of
-// `out_theta`: both buffers end up holding 8 KB of finished output in global-memory order, which
-// two TMA bulk stores then write (no LSU store traffic, every sector written once and in full).
+// Odd pass: lane l, row b fetches its parked even sample and stores the (even, odd) pair of theta
+// at e_theta[2 (l + 32 b)] and of phi at e_phi[2 (l + 32 b)]: 8 bytes per lane, 256 contiguous
+// bytes per instruction. The parked values come back in chunks of eight rows.
 template <bool HAS_EF>
-__device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], int lane, R *park, R *out_theta,
+__device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef,
                                          float &best, int &bb)
 {
-    static_for<0, 32>([&](auto bc) {
-        constexpr int b = decltype(bc)::value;
+    static_for<0, 4>([&](auto cc) {
+        constexpr int c = decltype(cc)::value;
+        unsigned long long ev[8];
         if (HAS_EF) {
-            float ot, op, et, ep;
-            L::unpack(zr[b], ot, op);
-            L::unpack(park[b * 32 + lane], et, ep);
-            out_theta[b * 32 + lane] = L::pack(et, ot);
-            park[b * 32 + lane] = L::pack(ep, op);
+            static_for<0, 8>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                ev[j] = tmem_ld64(tpark + 2 * (8 * c + j));
+            });
+            tmem_wait_ld(ev);
         }
-        R q = L::mul(zr[b], zr[b]);
-        q = L::fma(zi[b], zi[b], q);
-        float qt, qp;
-        L::unpack(q, qt, qp);
-        const float e2 = qt + qp;
-        if (e2 > best) { best = e2; bb = b; }
+        static_for<0, 8>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            constexpr int b = 8 * c + j;
+            if (HAS_EF) {
+                float ot, op, et, ep;
+                L::unpack(zr[b], ot, op);
+                R e; e.v = ev[j];
+                L::unpack(e, et, ep);
+                st_global_b64(ef + 2 * (lane + 32 * b), L::pack(et, ot));
+                st_global_b64(ef + 2 * kM + 2 * (lane + 32 * b), L::pack(ep, op));
+            }
+            R q = L::mul(zr[b], zr[b]);
+            q = L::fma(zi[b], zi[b], q);
+            float qt, qp;
+            L::unpack(q, qt, qp);
+            const float e2 = qt + qp;
+            if (e2 > best) { best = e2; bb = b; }
+        });
     });
 }
 
-// Shared-memory footprint of one instantiation.
+// Per-instantiation geometry: shared memory per warp, tensor-memory columns per warp, warps per CTA.
 template <int K2LO, int K2HI>
 struct W32Geom {
     static constexpr int kBandRows = K2HI - K2LO + 1;
@@ -173,23 +195,31 @@ struct W32Geom {
     static constexpr int kMirLo = 31 - K2HI;
     static constexpr int kMirHi = (32 - K2LO) > 31 ? 31 : (32 - K2LO);
     static constexpr int kMirRows = kMirHi - kMirLo + 1;
-    // the stash region doubles as the odd transform's transpose buffer (the even samples are
-    // parked in X by then), so it is at least as large as X
-    static constexpr int kStashBytes = kBandRows * 512 > kXBytes ? kBandRows * 512 : kXBytes;
-    static constexpr int kWarpBytes =
-        (kXBytes + kStashBytes) > kMirRows * 512 ? (kXBytes + kStashBytes) : kMirRows * 512;
+    // one buffer per warp: the padded 32x32 transpose plane, reused for the mirror exchange
+    // (two planes of kMirRows x 32 packed values)
+    static constexpr int kWarpBytes = kXBytes > kMirRows * 512 ? kXBytes : kMirRows * 512;
+    // tensor-memory columns (32-bit, per lane): stash of E, 4 per band row, then the parked even samples
+    static constexpr int kStashCols = 4 * kBandRows;
+    static constexpr int kParkCol = kStashCols;
+    static constexpr int kCols = kStashCols + 64;
+    // warps of one scheduler share that scheduler's 32 TMEM lanes, so they split the 512 columns
+    static constexpr int kWarps = 3 * kCols <= 512 ? 12 : 8;
+    static constexpr int kColStride = 512 / (kWarps / 4);
+    static_assert(kCols <= kColStride, "tensor-memory columns per warp");
 };
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM>
-__global__ void __launch_bounds__(kWarps * 32, 1)
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, bool TIGHT>
+__global__ void __launch_bounds__(W32Geom<K2LO, K2HI>::kWarps * 32, 1)
 unfold_w32_kernel(W32Params p)
 {
     using G = W32Geom<K2LO, K2HI>;
+    constexpr int kWarps = G::kWarps;
     extern __shared__ __align__(128) unsigned char smem[];
     float2 *T = reinterpret_cast<float2 *>(smem);               // [32][32] pass twiddles
     float2 *TS = T + 1024;                                       // [1024] W_2048^k
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + kTabBytes);     // [2] Minv slot filled
     int *done = reinterpret_cast<int *>(smem + kTabBytes + 16);          // [2] warps finished with the slot
+    uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabBytes + 32);
     const uint32_t minv_bytes = (uint32_t)p.K * 32u;
     const uint32_t slot_bytes = MINV_SMEM ? ((minv_bytes + 127u) & ~127u) : 0u;
     unsigned char *mslot = smem + kTabBytes + kCtlBytes;
@@ -198,16 +228,16 @@ unfold_w32_kernel(W32Params p)
     const int lane = threadIdx.x & 31;
     unsigned char *wbase = mslot + 2 * (size_t)slot_bytes + (size_t)warp * G::kWarpBytes;
     R *X = reinterpret_cast<R *>(wbase);                         // transpose buffer
-    float4 *Q = reinterpret_cast<float4 *>(wbase);               // mirror exchange (overlays X + stash)
-    float4 *ST = reinterpret_cast<float4 *>(wbase + kXBytes);    // stash [row][lane] (re, im) packed
-    R *X2 = reinterpret_cast<R *>(wbase + kXBytes);              // second transpose buffer (overlays the stash)
+    R *QA = X;                                                   // mirror exchange, real plane
+    R *QB = X + G::kMirRows * 32;                                // mirror exchange, imaginary plane
 
     const long S = p.n_stations;
     const long u0 = p.n_units * (long)blockIdx.x / (long)gridDim.x;
     const long u1 = p.n_units * ((long)blockIdx.x + 1) / (long)gridDim.x;
-    if (u1 <= u0) return;
-    const long e0 = u0 / S, e1 = (u1 - 1) / S;
+    // (no early exit: every CTA allocates and frees tensor memory; an empty range skips the loops)
+    const long e0 = u0 / S, e1 = u1 > u0 ? (u1 - 1) / S : e0 - 1;
 
+    if (warp == 0) tmem_alloc_all(tmem_base);
     if (MINV_SMEM && threadIdx.x == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
@@ -222,7 +252,12 @@ unfold_w32_kernel(W32Params p)
         T[i] = p.tw1024[(k1 * t) & 1023];
         TS[i] = p.twN[i];
     }
+    tmem_fence_before_sync();
     __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tbase = *tmem_base;
+    const uint32_t tstash = tmem_addr(tbase, warp, (warp >> 2) * G::kColStride);
+    const uint32_t tpark = tstash + G::kParkCol;
 
 #pragma unroll 1
     for (long e = e0; e <= e1; ++e) {
@@ -250,102 +285,115 @@ unfold_w32_kernel(W32Params p)
                 B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
             });
 
-            // ---- a2: forward FFT of g_0, g_1
-            fft32<L>(A, B);
-            pass_twiddle(A, B, T, lane);
-            if (HAS_EF) { // the previous station's bulk stores must have read X / X2 before they are reused
-                if (lane == 0) bulk_wait_group_read0();
-                __syncwarp();
-            }
-            transpose_plane(A, X, lane);
-            transpose_plane(B, X, lane);
-            fft32<L>(A, B);
-
-            // ---- mirror exchange: publish the rows that are somebody's bin 1024-k
-            static_for<G::kMirLo, G::kMirHi + 1>([&](auto rc) {
-                constexpr int r = decltype(rc)::value;
-                float ax, ay, bx, by;
-                L::unpack(A[r], ax, ay); L::unpack(B[r], bx, by);
-                Q[(r - G::kMirLo) * 32 + lane] = make_float4(ax, ay, bx, by);
-            });
-            __syncwarp();
-            if (!minv_ready) { mbar_wait(&full[slot], parity); minv_ready = true; }
-
-            // ---- separate channels, fold the two polyphase halves, a4: E = Minv V
-            R Zr[32], Zi[32]; // inverse-transform input, element k2 at brev5(k2)
-            static_for<0, 32>([&](auto kc) {
-                constexpr int k2 = decltype(kc)::value;
-                R er = L::zero(), ei = L::zero();
-                if constexpr (k2 >= K2LO && k2 <= K2HI) {
-                    const int k = lane + 32 * k2;
-                    if (k >= p.k_lo && k <= p.k_hi) {
-                        // partner bin 1024-k lives in lane (32-lane)&31, row 31-k2 (row 32-k2 for lane 0)
-                        // (k = 0, whose partner row would be 32, is never in band: k_lo >= 1)
-                        const int prow = (lane == 0 ? 32 - k2 : 31 - k2) - G::kMirLo;
-                        const float4 pq = Q[prow * 32 + ((32 - lane) & 31)];
-                        const R pr = L::pack(pq.x, pq.y), pi = L::pack(pq.z, pq.w);
-                        // F'_0 = G + conj(Gm) = 2 FFT(v0 polyphase r), F'_1 = -i (G - conj(Gm)) = 2 FFT(v1 polyphase r)
-                        const R f0r = L::add(A[k2], pr), f0i = L::sub(B[k2], pi);
-                        const R f1r = L::add(B[k2], pi), f1i = L::sub(pr, A[k2]);
-                        float f0r0, f0r1, f0i0, f0i1, f1r0, f1r1, f1i0, f1i1;
-                        L::unpack(f0r, f0r0, f0r1); L::unpack(f0i, f0i0, f0i1);
-                        L::unpack(f1r, f1r0, f1r1); L::unpack(f1i, f1i0, f1i1);
-                        const float2 w = TS[k]; // W_2048^k = (wr, wi)
-                        // 2 V_c = F'_c(r=0) + W F'_c(r=1)
-                        float v0r = fmaf(w.x, f0r1, f0r0); v0r = fmaf(-w.y, f0i1, v0r);
-                        float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
-                        float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
-                        float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
-                        const float4 m0 = MINV_SMEM ? MA[k - p.k_lo] : ld_nc_f4(MA + (k - p.k_lo));
-                        const float4 m1 = MINV_SMEM ? MB[k - p.k_lo] : ld_nc_f4(MB + (k - p.k_lo));
-                        const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
-                        er = L::mul(Ma, L::bc(v0r)); er = L::fma(Mb, L::bc(-v0i), er);
-                        er = L::fma(Mc, L::bc(v1r), er); er = L::fma(Md, L::bc(-v1i), er);
-                        ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
-                        ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
+            // ---- three 1024-point transforms through ONE copy of the FFT code (the instruction
+            // stream of a fully unrolled station is ~90 KB, far beyond the instruction caches; with
+            // twelve warps at different places in it, instruction fetch was the first limiter):
+            //   t = 0 forward (A = Re, B = Im); t = 1, 2 inverse, which is the forward routine with
+            //   the roles swapped (A = Im, B = Re).
+            float best0 = -1.0f, best1 = -1.0f; int b0 = 0, b1 = 0;
+#pragma unroll 1
+            for (int t = 0; t < 3; ++t) {
+#pragma unroll 1
+                for (int h = 0; h < 2; ++h) {
+                    fft32<L>(A, B);
+                    if (h == 0) {
+                        pass_twiddle(A, B, T, lane);
+                        transpose_plane(A, X, lane);
+                        transpose_plane(B, X, lane);
                     }
                 }
-                Zr[brev5(k2)] = er; Zi[brev5(k2)] = ei;
-            });
-            __syncwarp(); // all mirror reads done before the stash overwrites the region
+                if (t == 0) {
+                    // ---- a2 done. Mirror exchange: publish the rows that are somebody's bin 1024-k
+                    static_for<G::kMirLo, G::kMirHi + 1>([&](auto rc) {
+                        constexpr int r = decltype(rc)::value;
+                        QA[(r - G::kMirLo) * 32 + lane] = A[r];
+                        QB[(r - G::kMirLo) * 32 + lane] = B[r];
+                    });
+                    __syncwarp();
+                    if (!minv_ready) { mbar_wait(&full[slot], parity); minv_ready = true; }
 
-            // ---- stash E for the odd-sample transform
-            static_for<K2LO, K2HI + 1>([&](auto kc) {
-                constexpr int k2 = decltype(kc)::value;
-                float a, b, c, d;
-                L::unpack(Zr[brev5(k2)], a, b); L::unpack(Zi[brev5(k2)], c, d);
-                ST[(k2 - K2LO) * 32 + lane] = make_float4(a, b, c, d);
-            });
+                    // ---- separate channels, fold the two polyphase halves, a4: E = Minv V
+                    R Zr[32], Zi[32]; // inverse-transform input, element k2 at brev5(k2)
+                    static_for<0, 32>([&](auto kc) {
+                        constexpr int k2 = decltype(kc)::value;
+                        R er = L::zero(), ei = L::zero();
+                        if constexpr (k2 >= K2LO && k2 <= K2HI) {
+                            const int k = lane + 32 * k2;
+                            // interior rows of a tight band are in band by construction
+                            constexpr bool kEdge = !TIGHT || k2 == K2LO || k2 == K2HI;
+                            if (!kEdge || (k >= p.k_lo && k <= p.k_hi)) {
+                                // partner bin 1024-k lives in lane (32-lane)&31, row 31-k2 (row 32-k2 for lane 0)
+                                // (k = 0, whose partner row would be 32, is never in band: k_lo >= 1)
+                                const int prow = (lane == 0 ? 32 - k2 : 31 - k2) - G::kMirLo;
+                                const R pr = QA[prow * 32 + ((32 - lane) & 31)];
+                                const R pi = QB[prow * 32 + ((32 - lane) & 31)];
+                                // F'_0 = G + conj(Gm) = 2 FFT(v0 polyphase r), F'_1 = -i (G - conj(Gm)) = 2 FFT(v1 polyphase r)
+                                const R f0r = L::add(A[k2], pr), f0i = L::sub(B[k2], pi);
+                                const R f1r = L::add(B[k2], pi), f1i = L::sub(pr, A[k2]);
+                                float f0r0, f0r1, f0i0, f0i1, f1r0, f1r1, f1i0, f1i1;
+                                L::unpack(f0r, f0r0, f0r1); L::unpack(f0i, f0i0, f0i1);
+                                L::unpack(f1r, f1r0, f1r1); L::unpack(f1i, f1i0, f1i1);
+                                const float2 w = TS[k]; // W_2048^k = (wr, wi)
+                                // 2 V_c = F'_c(r=0) + W F'_c(r=1)
+                                float v0r = fmaf(w.x, f0r1, f0r0); v0r = fmaf(-w.y, f0i1, v0r);
+                                float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
+                                float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
+                                float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
+                                const float4 m0 = MINV_SMEM ? MA[k - p.k_lo] : ld_nc_f4(MA + (k - p.k_lo));
+                                const float4 m1 = MINV_SMEM ? MB[k - p.k_lo] : ld_nc_f4(MB + (k - p.k_lo));
+                                const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
+                                er = L::mul(Ma, L::bc(v0r)); er = L::fma(Mb, L::bc(-v0i), er);
+                                er = L::fma(Mc, L::bc(v1r), er); er = L::fma(Md, L::bc(-v1i), er);
+                                ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
+                                ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
+                            }
+                            // ---- stash E for the odd-sample transform (this lane's own tensor-memory columns)
+                            tmem_st64(tstash + 4 * (k2 - K2LO), er.v);
+                            tmem_st64(tstash + 4 * (k2 - K2LO) + 2, ei.v);
+                        }
+                        Zr[brev5(k2)] = er; Zi[brev5(k2)] = ei;
+                    });
+                    __syncwarp(); // all mirror reads done before the buffer becomes the transpose plane again
+                    // ---- a5: even samples  z[2m] = IFFT_1024(E): inverse roles, A = Im, B = Re
+                    static_for<0, 32>([&](auto ic) {
+                        constexpr int i = decltype(ic)::value;
+                        A[i] = Zi[i]; B[i] = Zr[i];
+                    });
+                } else if (t == 1) {
+                    emit_even<HAS_EF>(B, A, tpark, best0, b0);
+                    tmem_wait_st(); // stash and parked samples are in tensor memory
 
-            // ---- a5/a6: even samples  z[2m] = IFFT_1024(E)
-            float best0 = -1.0f, best1 = -1.0f; int b0 = 0, b1 = 0;
-            fft1024(Zi, Zr, X, T, lane);
-            emit_even<HAS_EF>(Zr, Zi, lane, X, best0, b0);
-
-            // ---- odd samples  z[2m+1] = IFFT_1024(E W_2048^-k)
-            static_for<0, 32>([&](auto kc) {
-                constexpr int k2 = decltype(kc)::value;
-                R er = L::zero(), ei = L::zero();
-                if constexpr (k2 >= K2LO && k2 <= K2HI) {
-                    const float4 s = ST[(k2 - K2LO) * 32 + lane];
-                    const float2 w = TS[lane + 32 * k2];
-                    const R sr = L::pack(s.x, s.y), si = L::pack(s.z, s.w);
-                    // (sr + i si)(wr - i wi)
-                    er = L::mul(sr, L::bc(w.x)); er = L::fma(si, L::bc(w.y), er);
-                    ei = L::mul(si, L::bc(w.x)); ei = L::fma(sr, L::bc(-w.y), ei);
-                }
-                Zr[brev5(k2)] = er; Zi[brev5(k2)] = ei;
-            });
-            __syncwarp(); // stash consumed by every lane before its region becomes the transpose buffer
-            fft1024(Zi, Zr, X2, T, lane);   // X holds the parked even samples
-            emit_odd<HAS_EF>(Zr, Zi, lane, X, X2, best1, b1);
-            if (HAS_EF) {
-                fence_proxy_async_smem(); // this lane's shared-memory writes -> visible to the TMA engine
-                __syncwarp();
-                if (lane == 0) {
-                    tma_bulk_s2g(ef, X2, kM * 8);           // e_theta[0..2048)
-                    tma_bulk_s2g(ef + 2 * kM, X, kM * 8);   // e_phi[0..2048)
-                    bulk_commit_group();
+                    // ---- odd samples  z[2m+1] = IFFT_1024(E W_2048^-k)
+                    static_for<0, 32>([&](auto kc) {
+                        constexpr int k2 = decltype(kc)::value;
+                        if constexpr (k2 < K2LO || k2 > K2HI) { A[brev5(k2)] = L::zero(); B[brev5(k2)] = L::zero(); }
+                    });
+                    constexpr int kChunks = (G::kBandRows + 3) / 4;
+                    static_for<0, kChunks>([&](auto cc) {
+                        constexpr int c = decltype(cc)::value;
+                        unsigned long long sv[8];
+                        static_for<0, 4>([&](auto jc) {
+                            constexpr int j = decltype(jc)::value;
+                            constexpr int row = 4 * c + j < G::kBandRows ? 4 * c + j : G::kBandRows - 1; // tail: re-read the last row
+                            sv[2 * j] = tmem_ld64(tstash + 4 * row);
+                            sv[2 * j + 1] = tmem_ld64(tstash + 4 * row + 2);
+                        });
+                        tmem_wait_ld(sv);
+                        static_for<0, 4>([&](auto jc) {
+                            constexpr int j = decltype(jc)::value;
+                            if constexpr (4 * c + j < G::kBandRows) {
+                                constexpr int k2 = K2LO + 4 * c + j;
+                                const float2 w = TS[lane + 32 * k2];
+                                R sr, si; sr.v = sv[2 * j]; si.v = sv[2 * j + 1];
+                                // (sr + i si)(wr - i wi)
+                                R er = L::mul(sr, L::bc(w.x)); er = L::fma(si, L::bc(w.y), er);
+                                R ei = L::mul(si, L::bc(w.x)); ei = L::fma(sr, L::bc(-w.y), ei);
+                                B[brev5(k2)] = er; A[brev5(k2)] = ei;
+                            }
+                        });
+                    });
+                } else {
+                    emit_odd<HAS_EF>(B, A, lane, tpark, ef, best1, b1);
                 }
             }
 
@@ -384,26 +432,30 @@ unfold_w32_kernel(W32Params p)
             }
         }
     }
-    if (HAS_EF && lane == 0) bulk_wait_group0(); // shared memory must outlive the last bulk stores
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_free_all(tbase);
 }
 
 template <int K2LO, int K2HI, bool MINV_SMEM>
 size_t w32_smem_bytes(int K)
 {
+    using G = W32Geom<K2LO, K2HI>;
     const size_t slot = MINV_SMEM ? (((size_t)K * 32 + 127) & ~(size_t)127) : 0;
-    return (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)kWarps * W32Geom<K2LO, K2HI>::kWarpBytes;
+    return (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)G::kWarps * G::kWarpBytes;
 }
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM>
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, bool TIGHT>
 cudaError_t launch_inst(const W32Params &q, cudaStream_t s)
 {
+    using G = W32Geom<K2LO, K2HI>;
     const size_t smem = w32_smem_bytes<K2LO, K2HI, MINV_SMEM>(q.K);
-    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM>;
+    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, TIGHT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    long grid = (q.n_units + kWarps - 1) / kWarps;
+    long grid = (q.n_units + G::kWarps - 1) / G::kWarps;
     if (grid > 148) grid = 148;
-    kern<<<(unsigned)grid, kWarps * 32, smem, s>>>(q);
+    kern<<<(unsigned)grid, G::kWarps * 32, smem, s>>>(q);
     return cudaGetLastError();
 }
 
@@ -426,9 +478,9 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     cudaError_t e;
     if ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) // configs[1]: 30-80 MHz at fs = 180 MHz
-        e = efield ? launch_inst<10, 28, true, true>(q, s) : launch_inst<10, 28, false, true>(q, s);
+        e = efield ? launch_inst<10, 28, true, true, true>(q, s) : launch_inst<10, 28, false, true, true>(q, s);
     else
-        e = efield ? launch_inst<0, 31, true, false>(q, s) : launch_inst<0, 31, false, false>(q, s);
+        e = efield ? launch_inst<0, 31, true, false, false>(q, s) : launch_inst<0, 31, false, false, false>(q, s);
     count_launches(1);
     return e;
 }
