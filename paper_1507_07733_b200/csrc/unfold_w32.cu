@@ -291,17 +291,22 @@ unfold_w32_kernel(W32Params p)
             //   t = 0 forward (A = Re, B = Im); t = 1, 2 inverse, which is the forward routine with
             //   the roles swapped (A = Im, B = Re).
             float best0 = -1.0f, best1 = -1.0f; int b0 = 0, b1 = 0;
+            // (Loops are written so that each exit leaves straight from the FFT: a join of the
+            // "continue" and "exit" paths would cost a register shuffle on every pass.)
+            int t = 0;
 #pragma unroll 1
-            for (int t = 0; t < 3; ++t) {
+            for (;;) {
+                bool second = false;
 #pragma unroll 1
-                for (int h = 0; h < 2; ++h) {
+                for (;;) {
                     fft32<L>(A, B);
-                    if (h == 0) {
-                        pass_twiddle(A, B, T, lane);
-                        transpose_plane(A, X, lane);
-                        transpose_plane(B, X, lane);
-                    }
+                    if (second) break;
+                    pass_twiddle(A, B, T, lane);
+                    transpose_plane(A, X, lane);
+                    transpose_plane(B, X, lane);
+                    second = true;
                 }
+                if (t == 2) break;
                 if (t == 0) {
                     // ---- a2 done. Mirror exchange: publish the rows that are somebody's bin 1024-k
                     static_for<G::kMirLo, G::kMirHi + 1>([&](auto rc) {
@@ -359,7 +364,7 @@ unfold_w32_kernel(W32Params p)
                         constexpr int i = decltype(ic)::value;
                         A[i] = Zi[i]; B[i] = Zr[i];
                     });
-                } else if (t == 1) {
+                } else {
                     emit_even<HAS_EF>(B, A, tpark, best0, b0);
                     tmem_wait_st(); // stash and parked samples are in tensor memory
 
@@ -392,10 +397,10 @@ unfold_w32_kernel(W32Params p)
                             }
                         });
                     });
-                } else {
-                    emit_odd<HAS_EF>(B, A, lane, tpark, ef, best1, b1);
                 }
+                ++t;
             }
+            emit_odd<HAS_EF>(B, A, lane, tpark, ef, best1, b1);
 
             // ---- a6: lane result (lowest index on ties), then warp argmax with the same rule
             float best = best0; int bi = 2 * (lane + 32 * b0);
