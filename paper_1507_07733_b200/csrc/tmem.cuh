@@ -48,18 +48,13 @@ __device__ __forceinline__ unsigned long long tmem_ld64(uint32_t addr)
                  "tcgen05.ld.sync.aligned.32x32b.x2.b32 {lo, hi}, [%1];\nmov.b64 %0, {lo, hi};\n}" : "=l"(v) : "r"(addr) : "memory");
     return v;
 }
-// Results of earlier tmem_ld64 calls may be used only after this. The loaded values are passed
-// through as in/out operands so the compiler cannot schedule a consumer above the wait.
+// Results of earlier tmem_ld64 calls may be used only after tmem_wait_ld(). The compiler does not
+// know that, so each loaded value is then passed through tmem_ld_dep(): an empty volatile asm that
+// "rewrites" it. Volatile asms keep their order, so no consumer can be scheduled above the wait.
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void tmem_wait_ld(unsigned long long (&v)[N])
+__device__ __forceinline__ void tmem_ld_dep(unsigned long long &a, unsigned long long &b)
 {
-    static_assert(N == 4 || N == 8, "chunk sizes used by the kernels");
-    if constexpr (N == 8)
-        asm volatile("tcgen05.wait::ld.sync.aligned;"
-                     : "+l"(v[0]), "+l"(v[1]), "+l"(v[2]), "+l"(v[3]), "+l"(v[4]), "+l"(v[5]), "+l"(v[6]), "+l"(v[7]) :: "memory");
-    else
-        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(v[0]), "+l"(v[1]), "+l"(v[2]), "+l"(v[3]) :: "memory");
+    asm volatile("" : "+l"(a), "+l"(b) :: "memory");
 }
 // Earlier tmem_st64 calls of this thread are complete (visible to its later tmem_ld64).
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
