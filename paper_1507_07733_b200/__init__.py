@@ -4,4 +4,4 @@ The product is the CUDA library libaera_unfold.so (csrc/, C ABI in include/aera_
 `binding` is the thin ctypes layer with the same entry-point names; importing it loads the
 library and fails loudly if it cannot be built or loaded. There is no CPU fallback.
 """
-__all__ = ["binding", "build"]
+__all__ = ["binding", "build", "sharding"]
