@@ -242,7 +242,10 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int K, long n_dirs, int n_sta
     w.off_minv = o; o = align_up(o + (size_t)n_dirs * K * 4 * cb);
     w.off_scratch = o; o = align_up(o + generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations));
     w.off_spectra = o;
-    if (op == AERA_OP_SCAN) o = align_up(o + generic_scan_spectra_bytes(dtype, K, n_stations));
+    if (op == AERA_OP_SCAN) { // room for either scan path's station spectra
+        size_t a = generic_scan_spectra_bytes(dtype, K, n_stations), b = scan_w32_spectra_bytes(n_stations);
+        o = align_up(o + (a > b ? a : b));
+    }
     w.total = o > 0 ? o : kAlign;
     return w;
 }
@@ -431,11 +434,15 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
 
+    const bool warp_path = kernel_variant() == 0 && scan_w32_supported(dtype, pl->dev);
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_dirs, ws + w.off_minv,
-                                MINV_ROWS, 2.0 / (double)n_samples, s);
+                                warp_path ? MINV_PACKED : MINV_ROWS, (warp_path ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
-    e = launch_scan_generic(dtype, pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx,
-                            ws + w.off_spectra, ws + w.off_scratch, s);
+    if (warp_path)
+        e = launch_scan_w32(pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx, ws + w.off_spectra, s);
+    else
+        e = launch_scan_generic(dtype, pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx,
+                                ws + w.off_spectra, ws + w.off_scratch, s);
     if (e != cudaSuccess) return cuda_fail(e, "scan kernel launch");
     return AERA_OK;
 }

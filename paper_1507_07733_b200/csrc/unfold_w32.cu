@@ -36,21 +36,10 @@
 //
 // The in-band rows (bins k = lane + 32 row) are template parameters, so every per-row decision is
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
-#include "aera_internal.h"
-#include "async_copy.cuh"
-#include "fft32.cuh"
-#include "tmem.cuh"
+#include "w32_common.cuh"
 
 namespace aera {
 namespace {
-
-using L = LaneF32x2;
-using R = F2;
-
-constexpr int kM = 1024;
-constexpr int kXBytes = 33 * 32 * 8;   // padded 32x32 transpose buffer, 8-byte elements
-constexpr int kTabBytes = 2 * 1024 * 8; // T + TS
-constexpr int kCtlBytes = 128;          // mbarriers + counters + TMEM base address
 
 struct W32Params {
     const float *traces;
@@ -63,157 +52,6 @@ struct W32Params {
     long n_units;
     int n_stations;
     int k_lo, k_hi, K;
-};
-
-__device__ __forceinline__ R ld_stream_b64(const void *p)
-{
-    R r;
-    asm volatile("ld.global.nc.L1::no_allocate.b64 %0, [%1];" : "=l"(r.v) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ float4 ld_nc_f4(const float4 *p)
-{
-    float4 r;
-    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-}
-
-// y[k1] *= W_1024^(k1 * lane) ; T[k1*32 + lane] holds the twiddle (re, im). "A" plays the real part.
-__device__ __forceinline__ void pass_twiddle(R (&A)[32], R (&B)[32], const float2 *__restrict__ T, int lane)
-{
-    static_for<1, 32>([&](auto kc) {
-        constexpr int k1 = decltype(kc)::value;
-        const float2 w = T[k1 * 32 + lane];
-        const R wr = L::bc(w.x), wi = L::bc(w.y), nwi = L::bc(-w.y);
-        R a = L::mul(A[k1], wr);
-        a = L::fma(B[k1], nwi, a);
-        R b = L::mul(A[k1], wi);
-        b = L::fma(B[k1], wr, b);
-        A[k1] = a; B[k1] = b;
-    });
-}
-
-// 32x32 transpose of one register plane through the padded buffer: value k1 of lane t goes to lane
-// k1, which receives it as input element t of its second-pass FFT (stored at position brev5(t)).
-__device__ __forceinline__ void transpose_plane(R (&P)[32], R *X, int lane)
-{
-    static_for<0, 32>([&](auto kc) {
-        constexpr int k1 = decltype(kc)::value;
-        X[k1 * 33 + lane] = P[k1];
-    });
-    __syncwarp();
-    static_for<0, 32>([&](auto tc) {
-        constexpr int t = decltype(tc)::value;
-        P[brev5(t)] = X[lane * 33 + t];
-    });
-    __syncwarp();
-}
-
-// Full 1024-point forward FFT of the packed data held as in[brev5(j)] = x[lane + 32 j].
-// On return lane k1 holds X[k1 + 32 k2] in (A[k2], B[k2]). Call with (B, A) for the inverse.
-__device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const float2 *__restrict__ T, int lane)
-{
-    fft32<L>(A, B);
-    pass_twiddle(A, B, T, lane);
-    transpose_plane(A, X, lane);
-    transpose_plane(B, X, lane);
-    fft32<L>(A, B);
-}
-
-__device__ __forceinline__ void st_global_b64(void *p, R v)
-{
-    asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
-}
-
-// Outputs of one inverse transform: lane a, register b holds z[m = a + 32 b] of (theta, phi);
-// sample index n = 2 m + parity. Both routines track the maximum of env^2 over b (ascending,
-// strict >, so the lowest b wins ties).
-//
-// Even samples come out one whole inverse transform before the odd ones. Writing them straight to
-// global memory would fill only half of every 32-byte sector, and the half-written sectors get
-// evicted from L2 (ECC read-modify-write in DRAM: +35 % read, +13 % write traffic measured). So
-// the even pass parks Re z (theta, phi) in this lane's tensor-memory columns and the odd pass
-// stores (even, odd) pairs.
-template <bool HAS_EF>
-__device__ __forceinline__ void emit_even(const R (&zr)[32], const R (&zi)[32], uint32_t tpark, float &best, int &bb)
-{
-    static_for<0, 32>([&](auto bc) {
-        constexpr int b = decltype(bc)::value;
-        if (HAS_EF) tmem_st64(tpark + 2 * b, zr[b].v);
-        R q = L::mul(zr[b], zr[b]);
-        q = L::fma(zi[b], zi[b], q);
-        float qt, qp;
-        L::unpack(q, qt, qp);
-        const float e2 = qt + qp;
-        if (e2 > best) { best = e2; bb = b; }
-    });
-}
-
-// Odd pass: lane l, row b fetches its parked even sample and stores the (even, odd) pair of theta
-// at e_theta[2 (l + 32 b)] and of phi at e_phi[2 (l + 32 b)]: 8 bytes per lane, 256 contiguous
-// bytes per instruction. The parked values come back in chunks of eight rows.
-template <bool HAS_EF>
-__device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef,
-                                         float &best, int &bb)
-{
-    static_for<0, 4>([&](auto cc) {
-        constexpr int c = decltype(cc)::value;
-        unsigned long long ev[8];
-        if (HAS_EF) {
-            static_for<0, 8>([&](auto jc) {
-                constexpr int j = decltype(jc)::value;
-                ev[j] = tmem_ld64(tpark + 2 * (8 * c + j));
-            });
-            tmem_wait_ld();
-            static_for<0, 4>([&](auto jc) {
-                constexpr int j = decltype(jc)::value;
-                tmem_ld_dep(ev[2 * j], ev[2 * j + 1]);
-            });
-        }
-        static_for<0, 8>([&](auto jc) {
-            constexpr int j = decltype(jc)::value;
-            constexpr int b = 8 * c + j;
-            if (HAS_EF) {
-                float ot, op, et, ep;
-                L::unpack(zr[b], ot, op);
-                R e; e.v = ev[j];
-                L::unpack(e, et, ep);
-                st_global_b64(ef + 2 * (lane + 32 * b), L::pack(et, ot));
-                st_global_b64(ef + 2 * kM + 2 * (lane + 32 * b), L::pack(ep, op));
-            }
-            R q = L::mul(zr[b], zr[b]);
-            q = L::fma(zi[b], zi[b], q);
-            float qt, qp;
-            L::unpack(q, qt, qp);
-            const float e2 = qt + qp;
-            if (e2 > best) { best = e2; bb = b; }
-        });
-    });
-}
-
-// Per-instantiation geometry: shared memory per warp, tensor-memory columns per warp, warps per CTA.
-template <int K2LO, int K2HI>
-struct W32Geom {
-    static constexpr int kLo = K2LO, kHi = K2HI;
-    static constexpr int kBandRows = K2HI - K2LO + 1;
-    // rows that hold some band bin's mirror 1024-k: row 31-r for lanes >= 1, row 32-r for lane 0
-    static constexpr int kMirLo = 31 - K2HI;
-    static constexpr int kMirHi = (32 - K2LO) > 31 ? 31 : (32 - K2LO);
-    // rows of the forward spectrum published to shared memory: the band rows and their mirror rows
-    static constexpr int kPubLo = kMirLo < K2LO ? kMirLo : K2LO;
-    static constexpr int kPubHi = kMirHi > K2HI ? kMirHi : K2HI;
-    static constexpr int kPubRows = kPubHi - kPubLo + 1;
-    // one buffer per warp: the padded 32x32 transpose plane, reused for the published spectrum
-    // (two planes of kPubRows x 32 packed values)
-    static constexpr int kWarpBytes = kXBytes > kPubRows * 512 ? kXBytes : kPubRows * 512;
-    // tensor-memory columns (32-bit, per lane): stash of E, 4 per band row, then the parked even samples
-    static constexpr int kStashCols = 4 * kBandRows;
-    static constexpr int kParkCol = kStashCols;
-    static constexpr int kCols = kStashCols + 64;
-    // warps of one scheduler share that scheduler's 32 TMEM lanes, so they split the 512 columns
-    static constexpr int kWarps = 3 * kCols <= 512 ? 12 : 8;
-    static constexpr int kColStride = 512 / (kWarps / 4);
-    static_assert(kCols <= kColStride, "tensor-memory columns per warp");
 };
 
 // One band row per iteration: row k2 = kLo + r holds bin k = lane + 32 k2 of the packed forward
@@ -257,35 +95,6 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
         tmem_st64(tstash + 4 * r + 2, ei.v);
     }
 }
-
-// Input of one inverse transform, element k2 at position brev5(k2): E[k] (even samples) or
-// E[k] W_2048^-k (ODD) on the band rows, zero elsewhere. E comes back from tensor memory.
-template <class G, bool ODD>
-__device__ __forceinline__ void build_inverse_input(R (&Zr)[32], R (&Zi)[32], const float2 *TS, int lane, uint32_t tstash)
-{
-    static_for<0, 32>([&](auto kc) {
-        constexpr int k2 = decltype(kc)::value;
-        if constexpr (k2 < G::kLo || k2 > G::kHi) { Zr[brev5(k2)] = L::zero(); Zi[brev5(k2)] = L::zero(); }
-        else {
-            Zr[brev5(k2)].v = tmem_ld64(tstash + 4 * (k2 - G::kLo));
-            Zi[brev5(k2)].v = tmem_ld64(tstash + 4 * (k2 - G::kLo) + 2);
-        }
-    });
-    tmem_wait_ld();
-    static_for<G::kLo, G::kHi + 1>([&](auto kc) {
-        constexpr int k2 = decltype(kc)::value;
-        tmem_ld_dep(Zr[brev5(k2)].v, Zi[brev5(k2)].v);
-        if (ODD) {
-            const float2 w = TS[lane + 32 * k2];
-            const R sr = Zr[brev5(k2)], si = Zi[brev5(k2)];
-            // (sr + i si)(wr - i wi)
-            R er = L::mul(sr, L::bc(w.x)); er = L::fma(si, L::bc(w.y), er);
-            R ei = L::mul(si, L::bc(w.x)); ei = L::fma(sr, L::bc(-w.y), ei);
-            Zr[brev5(k2)] = er; Zi[brev5(k2)] = ei;
-        }
-    });
-}
-
 
 template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, bool TIGHT>
 __global__ void __launch_bounds__(W32Geom<K2LO, K2HI>::kWarps * 32, 1)

@@ -127,6 +127,25 @@ def test_config2_scan(B, orc, variant):
     assert rep.max_amp <= TOL["f32"]["amp"] and rep.idx_miss == 0, str(rep)
 
 
+def test_config2_scan_ragged_tiles(B, orc):
+    """Scan tiles are 4 stations x 3 directions: 7 stations x 10 directions leaves both tails ragged."""
+    wl = ai.WORKLOADS[2]
+    H = table_for(wl)
+    ev = ai.make_event(wl, 0)
+    tr = np.ascontiguousarray(ev.traces[5:12])
+    dirs = ai.scan_directions()[[3, 181, 400, 777, 1500, 2999, 3000, 5000, 7000, 7379]]
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        amp, idx = B.aera_scan_directions(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(dirs).cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+    finally:
+        pat.free()
+    oamp, oidx = orc.scan(wl.grid, H, wl.fs_hz, tr, dirs)
+    rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx)
+    print(f"\n[parity cfg2 scan ragged] {rep}")
+    assert rep.max_amp <= TOL["f32"]["amp"] and rep.idx_miss == 0, str(rep)
+
+
 # ------------------------------------------------------------------ sizes and edge cases
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("N", [64, 128, 256, 512, 1024, 2048, 4096, 8192])
