@@ -68,6 +68,11 @@ bool w32_supported(int dtype, const PlanDev &p);
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                               void *amp, int32_t *idx, const void *minv, cudaStream_t s);
 
+// ---- unfold_t4k_f64.cu: team-per-station kernel for N = 4096 fp64, band rows 4..12 (configs[3])
+bool t4k_f64_supported(int dtype, const PlanDev &p);
+cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s);
+
 // ---- scan_w32.cu: direction scan for N = 2048 fp32, band rows 10..28 (configs[2])
 bool scan_w32_supported(int dtype, const PlanDev &p);
 size_t scan_w32_spectra_bytes(int n_stations);

@@ -398,12 +398,15 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
     unsigned char *ws = static_cast<unsigned char *>(workspace);
 
     const bool warp_path = kernel_variant() == 0 && w32_supported(dtype, pl->dev);
-    // the warp kernel forms 2 V_c, so its matrix carries 1/N instead of 2/N
+    const bool team_path = kernel_variant() == 0 && t4k_f64_supported(dtype, pl->dev);
+    // the warp and team kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
-                                warp_path ? MINV_PACKED : MINV_ROWS, (warp_path ? 1.0 : 2.0) / (double)n_samples, s);
+                                warp_path ? MINV_PACKED : MINV_ROWS, ((warp_path || team_path) ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
+    else if (team_path)
+        e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
     else
         e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
                                   ws + w.off_minv, ws + w.off_scratch, s);

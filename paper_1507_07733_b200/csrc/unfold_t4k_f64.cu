@@ -1,0 +1,400 @@
+// Team-per-station fused unfolding kernel for N = 4096 fp64 (BASELINE configs[3]).
+//
+// A "team" of 4 warps (128 threads x 32 complex doubles = 128 registers each) holds one station
+// entirely in registers; a CTA runs 3 teams (12 warps, one CTA per SM, persistent). Every long
+// transform is 4096 = 4 x 1024: a radix-4 step across the team plus one 1024-point FFT per warp
+// (32 x 32 in registers with one shared-memory transpose, fft32.cuh with plain double lanes).
+//
+//   a1/a2 forward : g[n] = v0[n] + i v1[n] (two real transforms for one). Thread (warp w, lane)
+//                   loads g[m + 1024 j'], j' = 0..3, for its 8 values m = lane + 32 (8 w + jj) with
+//                   coalesced 8-byte loads, does the 4-point DFT over j' in registers (decimation in
+//                   frequency), multiplies y_q[m] by W_4096^{q m}; the team exchanges through shared
+//                   memory (lane-preserving, conflict-free) so that warp q owns y_q[0..1023], and
+//                   warp q's FFT_1024 gives G[4 k' + q].
+//   separation    : 2 V_0[k] = G[k] + conj G[N-k], 2 V_1[k] = -i (G[k] - conj G[N-k]); bin N-k lives
+//                   in warp (4-q)&3, so the mirror rows are published through shared memory.
+//   a4 solve      : (E_theta, E_phi)[k] = Minv[event][k] (2V_0, 2V_1)[k] on the band rows, in registers;
+//                   Minv = (1/N) H^-1 (pattern.cu, once per event) is read through L1/L2 (64 KB per
+//                   event at configs[3], shared by the event's 40 stations).
+//   a5 inverse    : the band holds at most one bin per residue k mod 1024 (K <= 1024), so
+//                   z[4 m + s] = IFFT_1024 over k' of E[k(k')] W_4096^{-s k(k')}: warp s does sample
+//                   phase s, first theta then phi. E crosses the team once through shared memory.
+//   a6 outputs    : e_p[n] = Re z_p[n] from registers; |z_theta|^2 waits in this lane's tensor-memory
+//                   columns (tmem.cuh) for |z_phi|^2; running (max, lowest index) per lane, warp
+//                   shuffle argmax, then the 4 warps of the team combine through shared memory.
+//
+// HBM traffic per station: 64 KB read once, 64 KB + 12 B written once.
+// The in-band rows (bins k = 4 (lane + 32 row) + q) are template parameters: <4, 12> is configs[3]
+// (k = 615..1638).
+#include "aera_internal.h"
+#include "async_copy.cuh"
+#include "fft32.cuh"
+#include "tmem.cuh"
+
+namespace aera {
+namespace {
+
+using LD = LaneF64;
+constexpr int kTeams = 3;
+constexpr int kTeamThreads = 128;
+constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane
+constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B: exchange / transposes / mirror rows / E_theta
+constexpr int kEStride = 260;                         // E buffer: slot = (k' & 3) * 260 + (k' >> 2), conflict-free both ways
+constexpr int kEPlane = 4 * kEStride;                 // doubles per plane
+constexpr int kRegionY = 2 * kEPlane * 8;             // 16 640 B: E_phi (re plane, im plane)
+constexpr int kTeamBytes = kRegionX + kRegionY;
+constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_4096^t, t < 1024)
+constexpr int kCtlF64 = 512;
+
+struct T4kParams {
+    const double *traces;
+    double *efield;
+    double *amp;
+    int32_t *idx;
+    const double2 *minv;   // [n_events][K][4] complex (MINV_ROWS), scaled by 1/N
+    const double2 *tw1024; // W_1024^m
+    const double2 *twN;    // W_4096^m
+    long n_units;
+    int n_stations;
+    int k_lo, k_hi, K;
+};
+
+__device__ __forceinline__ void team_sync(int team)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTeamThreads) : "memory");
+}
+__device__ __forceinline__ double ld_stream_f64(const double *p)
+{
+    double r;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double2 ld_nc_d2(const double2 *p)
+{
+    double2 r;
+    asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+
+// W_4096^t for any t in [0, 4096) from the first quadrant table: W^{t+1024} = -i W^t.
+__device__ __forceinline__ double2 w4096(const double2 *TQ, int t)
+{
+    const double2 w = TQ[t & 1023];
+    const int quad = (t >> 10) & 3;
+    double2 r;
+    r.x = (quad & 1) ? w.y : w.x;       // quad 1: -i w = (w.y, -w.x); quad 2: -w; quad 3: i w = (-w.y, w.x)
+    r.y = (quad & 1) ? -w.x : w.y;
+    if (quad & 2) { r.x = -r.x; r.y = -r.y; }
+    return r;
+}
+
+// y[k1] *= W_1024^(k1 * lane); "P" plays the real part.
+__device__ __forceinline__ void pass_twiddle_d(double (&P)[32], double (&Q)[32], const double2 *__restrict__ T, int lane)
+{
+    static_for<1, 32>([&](auto kc) {
+        constexpr int k1 = decltype(kc)::value;
+        const double2 w = T[k1 * 32 + lane];
+        double a = P[k1] * w.x; a = fma(Q[k1], -w.y, a);
+        double b = P[k1] * w.y; b = fma(Q[k1], w.x, b);
+        P[k1] = a; Q[k1] = b;
+    });
+}
+__device__ __forceinline__ void transpose_plane_d(double (&P)[32], double *X, int lane)
+{
+    static_for<0, 32>([&](auto kc) {
+        constexpr int k1 = decltype(kc)::value;
+        X[k1 * 33 + lane] = P[k1];
+    });
+    __syncwarp();
+    static_for<0, 32>([&](auto tc) {
+        constexpr int t = decltype(tc)::value;
+        P[brev5(t)] = X[lane * 33 + t];
+    });
+    __syncwarp();
+}
+// 1024-point forward FFT of in[brev5(j)] = x[lane + 32 j]; on return lane k1 holds X[k1 + 32 k2] in
+// (P[k2], Q[k2]). Call with (Q, P) for the un-normalised inverse. ONE copy of the 32-point code.
+__device__ __forceinline__ void fft1024_d(double (&P)[32], double (&Q)[32], double *X, const double2 *__restrict__ T, int lane)
+{
+    int second = 0;
+    asm volatile("" : "+r"(second));
+#pragma unroll 1
+    for (;;) {
+        fft32<LD>(P, Q);
+        if (second) break;
+        pass_twiddle_d(P, Q, T, lane);
+        transpose_plane_d(P, X, lane);
+        transpose_plane_d(Q, X, lane);
+        second = 1;
+        asm volatile("" : "+r"(second));
+    }
+}
+
+template <int RLO, int RHI, bool HAS_EF>
+__global__ void __launch_bounds__(kTeams *kTeamThreads, 1)
+unfold_t4k_f64_kernel(T4kParams p)
+{
+    constexpr int kRows = RHI - RLO + 1;            // band rows per thread
+    static_assert(kRows >= 1 && kRows <= 9, "band rows: K <= 1024 means at most 9 rows of 128 bins touch the band");
+    constexpr int kMirLo = 31 - RHI, kMirHi = (32 - RLO) > 31 ? 31 : (32 - RLO); // rows holding some band bin's mirror
+    constexpr int kMirRows = kMirHi - kMirLo + 1;
+    static_assert(4 * kMirRows * 512 <= kRegionX, "mirror rows fit region X");
+    extern __shared__ __align__(128) unsigned char smem[];
+    double2 *T = reinterpret_cast<double2 *>(smem);        // [32][32] pass twiddles W_1024^{k1 t}
+    double2 *TQ = T + 1024;                                 // W_4096^t, t < 1024
+    uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabF64);
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int team = warp >> 2, w = warp & 3;
+    double *peak_v = reinterpret_cast<double *>(smem + kTabF64 + 64) + team * 4;   // [team][4]
+    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + kTeams * 32) + team * 4;
+    unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kTeamBytes;
+    double *RX = reinterpret_cast<double *>(tb);            // region X
+    double *RY = reinterpret_cast<double *>(tb + kRegionX); // region Y
+    double *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
+
+    if (warp == 0) tmem_alloc_all(tmem_base);
+    for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
+        const int k1 = i >> 5, t = i & 31;
+        T[i] = p.tw1024[(k1 * t) & 1023];
+        TQ[i] = p.twN[i];
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tenv = tmem_addr(*tmem_base, warp, team * 64);  // |z_theta|^2, 2 columns per row
+
+    const long u0 = p.n_units * (long)blockIdx.x / (long)gridDim.x;
+    const long u1 = p.n_units * ((long)blockIdx.x + 1) / (long)gridDim.x;
+    constexpr int N = 4096;
+
+#pragma unroll 1
+    for (long u = u0 + team; u < u1; u += kTeams) {
+        const double *v = p.traces + (size_t)u * 2 * N;
+        double *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
+        const double2 *M = p.minv + (size_t)(u / p.n_stations) * p.K * 4;
+        if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(double));
+
+        double P[32], Q[32];
+        // ---- a1 + radix-4 step: thread holds y_q[m], q = 0..3, m = lane + 32 (8 w + jj), at [8 q + jj]
+        static_for<0, 8>([&](auto jc) {
+            constexpr int jj = decltype(jc)::value;
+            const int m = lane + 32 * (8 * w + jj);
+            const double x0r = ld_stream_f64(v + m), x1r = ld_stream_f64(v + m + 1024);
+            const double x2r = ld_stream_f64(v + m + 2048), x3r = ld_stream_f64(v + m + 3072);
+            const double x0i = ld_stream_f64(v + N + m), x1i = ld_stream_f64(v + N + m + 1024);
+            const double x2i = ld_stream_f64(v + N + m + 2048), x3i = ld_stream_f64(v + N + m + 3072);
+            const double ar = x0r + x2r, ai = x0i + x2i, br = x0r - x2r, bi = x0i - x2i;
+            const double cr = x1r + x3r, ci = x1i + x3i, dr = x1r - x3r, di = x1i - x3i;
+            P[jj] = ar + cr; Q[jj] = ai + ci;                    // y0
+            const double y1r = br + di, y1i = bi - dr;           // b - i d
+            const double y2r = ar - cr, y2i = ai - ci;
+            const double y3r = br - di, y3i = bi + dr;           // b + i d
+            const double2 w1 = TQ[m];                            // W_4096^m, m < 1024
+            const double2 w2 = w4096(TQ, 2 * m), w3 = w4096(TQ, 3 * m);
+            double t;
+            t = y1r * w1.x; P[8 + jj] = fma(y1i, -w1.y, t); t = y1r * w1.y; Q[8 + jj] = fma(y1i, w1.x, t);
+            t = y2r * w2.x; P[16 + jj] = fma(y2i, -w2.y, t); t = y2r * w2.y; Q[16 + jj] = fma(y2i, w2.x, t);
+            t = y3r * w3.x; P[24 + jj] = fma(y3i, -w3.y, t); t = y3r * w3.y; Q[24 + jj] = fma(y3i, w3.x, t);
+        });
+
+        // ---- team exchange: warp q collects y_q[lane + 32 j], j = 8 w' + jj, into FFT input order
+        team_sync(team);                                         // region X free (previous station done)
+        {
+            double *XB = RX;                                     // [q][j][lane]
+            static_for<0, 32>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;           // i = 8 q + jj
+                XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane] = P[i];
+            });
+            team_sync(team);
+            static_for<0, 32>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                P[brev5(j)] = XB[(w * 32 + j) * 32 + lane];
+            });
+            team_sync(team);
+            static_for<0, 32>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane] = Q[i];
+            });
+            team_sync(team);
+            static_for<0, 32>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                Q[brev5(j)] = XB[(w * 32 + j) * 32 + lane];
+            });
+            team_sync(team);
+        }
+        // ---- a2: warp q = w: G[4 (lane + 32 row) + q] in (P[row], Q[row])
+        fft1024_d(P, Q, XW, T, lane);
+        team_sync(team);                                         // all transposes done: region X becomes the mirror rows
+        {
+            double2 *PUB = reinterpret_cast<double2 *>(RX);      // [warp][mirror row][lane]
+            static_for<kMirLo, kMirHi + 1>([&](auto rc) {
+                constexpr int r = decltype(rc)::value;
+                PUB[(w * kMirRows + (r - kMirLo)) * 32 + lane] = make_double2(P[r], Q[r]);
+            });
+        }
+        team_sync(team);
+        // ---- separation + a4 on the band rows: E stays in registers until every mirror read is done
+        double Etr[kRows], Eti[kRows], Epr[kRows], Epi[kRows];
+        {
+            const double2 *PUB = reinterpret_cast<const double2 *>(RX);
+            const int pw = (4 - w) & 3;
+            const int plane = (w == 0) ? ((32 - lane) & 31) : (31 - lane);
+            const int padd = (w == 0 && lane == 0) ? 1 : 0;      // q = 0, lane 0: mirror row 32 - r
+            static_for<0, kRows>([&](auto rc) {
+                constexpr int i = decltype(rc)::value;
+                constexpr int r = RLO + i;
+                const int k = 4 * (lane + 32 * r) + w;
+                const bool inband = k >= p.k_lo && k <= p.k_hi;
+                int prow = 31 - r + padd;
+                prow = prow > kMirHi ? kMirHi : prow;
+                const double2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
+                int j = k - p.k_lo;
+                j = j < 0 ? 0 : (j > p.K - 1 ? p.K - 1 : j);
+                const double2 m0 = ld_nc_d2(M + 4 * j), m1 = ld_nc_d2(M + 4 * j + 1);
+                const double2 m2 = ld_nc_d2(M + 4 * j + 2), m3 = ld_nc_d2(M + 4 * j + 3);
+                const double v0r = P[r] + gm.x, v0i = Q[r] - gm.y;   // 2 V_0
+                const double v1r = Q[r] + gm.y, v1i = gm.x - P[r];   // 2 V_1
+                double er = m0.x * v0r; er = fma(-m0.y, v0i, er); er = fma(m1.x, v1r, er); er = fma(-m1.y, v1i, er);
+                double ei = m0.x * v0i; ei = fma(m0.y, v0r, ei); ei = fma(m1.x, v1i, ei); ei = fma(m1.y, v1r, ei);
+                double fr = m2.x * v0r; fr = fma(-m2.y, v0i, fr); fr = fma(m3.x, v1r, fr); fr = fma(-m3.y, v1i, fr);
+                double fi = m2.x * v0i; fi = fma(m2.y, v0r, fi); fi = fma(m3.x, v1i, fi); fi = fma(m3.y, v1r, fi);
+                Etr[i] = inband ? er : 0.0; Eti[i] = inband ? ei : 0.0;
+                Epr[i] = inband ? fr : 0.0; Epi[i] = inband ? fi : 0.0;
+            });
+        }
+        team_sync(team);                                         // mirror rows consumed: region X becomes E_theta
+        {
+            // residue slot of bin k = 4 (lane + 32 r) + q: q * 260 + lane + 32 (r & 7); rows r and r + 8
+            // share a slot and at most one of them is in band (K <= 1024); unused slots are zeroed.
+            double *ETr = RX, *ETi = RX + kEPlane, *EPr = RY, *EPi = RY + kEPlane;
+            static_for<0, 8>([&](auto cc) {
+                constexpr int c8 = decltype(cc)::value;
+                constexpr int r1 = RLO + ((c8 - RLO) & 7);       // first band row with r & 7 == c8
+                double a = 0.0, b = 0.0, c = 0.0, d = 0.0;
+                if constexpr (r1 <= RHI) { a = Etr[r1 - RLO]; b = Eti[r1 - RLO]; c = Epr[r1 - RLO]; d = Epi[r1 - RLO]; }
+                if constexpr (r1 + 8 <= RHI) { a += Etr[r1 + 8 - RLO]; b += Eti[r1 + 8 - RLO]; c += Epr[r1 + 8 - RLO]; d += Epi[r1 + 8 - RLO]; }
+                const int slot = w * kEStride + lane + 32 * c8;
+                ETr[slot] = a; ETi[slot] = b; EPr[slot] = c; EPi[slot] = d;
+            });
+        }
+        team_sync(team);
+
+        // ---- a5/a6: warp s = w produces samples n = 4 m + s; theta first, then phi
+        double best = -1.0; int bb = 0;
+        const int rslot = (lane & 3) * kEStride + (lane >> 2);
+#pragma unroll 1
+        for (int pol = 0; pol < 2; ++pol) {
+            const double *Er = pol ? RY : RX, *Ei = Er + kEPlane;
+            static_for<0, 32>([&](auto jc) {
+                constexpr int j = decltype(jc)::value;
+                P[brev5(j)] = Er[rslot + 8 * j];
+                Q[brev5(j)] = Ei[rslot + 8 * j];
+            });
+            if (w != 0) {                                        // E[k] W_4096^{-s k}, k = the band bin of residue k'
+                static_for<0, 32>([&](auto jc) {
+                    constexpr int j = decltype(jc)::value;
+                    const int kp = lane + 32 * j;
+                    const int k = kp + (((p.k_lo - kp + 1023) >> 10) << 10);
+                    const double2 tw = w4096(TQ, (w * k) & 4095);
+                    const double er = P[brev5(j)], ei = Q[brev5(j)];
+                    double a = er * tw.x; a = fma(ei, tw.y, a);
+                    double b = ei * tw.x; b = fma(er, -tw.y, b);
+                    P[brev5(j)] = a; Q[brev5(j)] = b;
+                });
+            }
+            if (pol == 0) team_sync(team);                       // everyone has E_theta before transposes reuse region X
+            fft1024_d(Q, P, XW, T, lane);                        // inverse: roles swapped
+            if (pol == 0) {
+                static_for<0, 32>([&](auto bc) {
+                    constexpr int b = decltype(bc)::value;
+                    if (HAS_EF) ef[4 * (lane + 32 * b) + w] = P[b];
+                    double e2 = P[b] * P[b]; e2 = fma(Q[b], Q[b], e2);
+                    tmem_st64(tenv + 2 * b, (unsigned long long)__double_as_longlong(e2));
+                });
+                tmem_wait_st();
+            } else {
+                static_for<0, 4>([&](auto cc) {
+                    constexpr int c = decltype(cc)::value;
+                    unsigned long long ev[8];
+                    static_for<0, 8>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        ev[j] = tmem_ld64(tenv + 2 * (8 * c + j));
+                    });
+                    tmem_wait_ld();
+                    static_for<0, 4>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        tmem_ld_dep(ev[2 * j], ev[2 * j + 1]);
+                    });
+                    static_for<0, 8>([&](auto jc) {
+                        constexpr int j = decltype(jc)::value;
+                        constexpr int b = 8 * c + j;
+                        if (HAS_EF) ef[N + 4 * (lane + 32 * b) + w] = P[b];
+                        double e2 = fma(P[b], P[b], __longlong_as_double((long long)ev[j]));
+                        e2 = fma(Q[b], Q[b], e2);
+                        if (e2 > best) { best = e2; bb = b; }
+                    });
+                });
+            }
+        }
+        // ---- a6: lane -> warp -> team argmax, lowest index on ties in every stage
+        int bi = 4 * (lane + 32 * bb) + w;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+        }
+        if (lane == 0) { peak_v[w] = best; peak_i[w] = bi; }
+        team_sync(team);
+        if (w == 0 && lane == 0) {
+            double bv = peak_v[0]; int bx = peak_i[0];
+#pragma unroll
+            for (int i = 1; i < 4; ++i)
+                if (peak_v[i] > bv || (peak_v[i] == bv && peak_i[i] < bx)) { bv = peak_v[i]; bx = peak_i[i]; }
+            p.amp[u] = sqrt(bv); p.idx[u] = bx;
+        }
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_free_all(*tmem_base);
+}
+
+template <int RLO, int RHI, bool HAS_EF>
+cudaError_t launch_t4k(const T4kParams &q, cudaStream_t s)
+{
+    const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * kTeamBytes;
+    auto kern = unfold_t4k_f64_kernel<RLO, RHI, HAS_EF>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    long grid = (q.n_units + kTeams - 1) / kTeams;
+    if (grid > 148) grid = 148;
+    kern<<<(unsigned)grid, kTeams * kTeamThreads, smem, s>>>(q);
+    return cudaGetLastError();
+}
+
+} // namespace
+
+bool t4k_f64_supported(int dtype, const PlanDev &p)
+{
+    // the one band geometry instantiated: rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3])
+    return dtype == AERA_F64 && p.N == 4096 && p.K <= 1024 && p.k_lo >= 1 && p.k_hi < 2048 &&
+           (p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12;
+}
+
+cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s)
+{
+    const long n_units = n_events * (long)n_stations;
+    if (n_units <= 0) return cudaSuccess;
+    ProfScope prof(KID_UNFOLD, s);
+    T4kParams q;
+    q.traces = (const double *)traces; q.efield = (double *)efield; q.amp = (double *)amp; q.idx = idx;
+    q.minv = (const double2 *)minv; q.tw1024 = (const double2 *)p.tw1024; q.twN = (const double2 *)p.twN;
+    q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
+    cudaError_t e = efield ? launch_t4k<4, 12, true>(q, s) : launch_t4k<4, 12, false>(q, s);
+    count_launches(1);
+    return e;
+}
+
+} // namespace aera
