@@ -48,7 +48,12 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
 //   MINV_ROWS   : complex entries (theta<-V0, theta<-V1, phi<-V0, phi<-V1)            (generic kernels)
 //   MINV_PACKED : per direction two planes A[K], B[K] of 4 reals: A = {t0.re, p0.re, t0.im, p0.im},
 //                 B = {t1.re, p1.re, t1.im, p1.im}                                     (warp kernels)
-enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1 };
+//   MINV_Q4     : per direction 16 planes [q = k & 3][entry 0..3 as in MINV_ROWS][C] complex, column
+//                 (k >> 2) - (k_lo >> 2), C = (k_hi >> 2) - (k_lo >> 2) + 1; slots of bins outside the
+//                 band are never written or used                                       (team kernel)
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2 };
+// complex elements per direction in the MINV_Q4 layout (<= 4 K + 32)
+__host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
                         const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s);
 size_t minv_smem_bytes(int dtype, int n_f);

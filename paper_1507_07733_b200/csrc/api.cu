@@ -239,7 +239,7 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int K, long n_dirs, int n_sta
     WsLayout w{};
     const size_t cb = cplx_bytes(dtype);
     size_t o = 0;
-    w.off_minv = o; o = align_up(o + (size_t)n_dirs * K * 4 * cb);
+    w.off_minv = o; o = align_up(o + (size_t)n_dirs * (K * 4 + 32) * cb); // + 32: MINV_Q4 plane padding
     w.off_scratch = o; o = align_up(o + generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations));
     w.off_spectra = o;
     if (op == AERA_OP_SCAN) { // room for either scan path's station spectra
@@ -401,7 +401,8 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
     const bool team_path = kernel_variant() == 0 && t4k_f64_supported(dtype, pl->dev);
     // the warp and team kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
-                                warp_path ? MINV_PACKED : MINV_ROWS, ((warp_path || team_path) ? 1.0 : 2.0) / (double)n_samples, s);
+                                warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : MINV_ROWS),
+                                ((warp_path || team_path) ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);

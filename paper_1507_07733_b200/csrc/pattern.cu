@@ -92,7 +92,7 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restrict__ dirs,
             const int *__restrict__ bin_if, const double *__restrict__ bin_tf, int K, double scale,
-            int layout, cx<T> *__restrict__ minv)
+            int layout, int k_lo, cx<T> *__restrict__ minv)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
@@ -152,6 +152,10 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         mp1.re = (T)(hr[0] * ir - hi[0] * ii);    mp1.im = (T)(hr[0] * ii + hi[0] * ir);
         if (layout == MINV_ROWS) {
             o[0] = mt0; o[1] = mt1; o[2] = mp0; o[3] = mp1;
+        } else if (layout == MINV_Q4) {
+            const int k = k_lo + j, C = ((k_lo + K - 1) >> 2) - (k_lo >> 2) + 1;
+            cx<T> *q = minv + (size_t)d * 16 * C + (size_t)(k & 3) * 4 * C + ((k >> 2) - (k_lo >> 2));
+            q[0] = mt0; q[C] = mt1; q[2 * C] = mp0; q[3 * C] = mp1;
         } else { // MINV_PACKED: two planes per direction, (theta, phi) side by side so a packed
                  // f32x2 load yields both: A[j] = {t0.re, p0.re, t0.im, p0.im}, B[j] = {t1.re, p1.re, t1.im, p1.im}
             cx<T> *a = minv + (size_t)d * K * 4 + (size_t)j * 2, *b = a + (size_t)K * 2;
@@ -178,12 +182,12 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
         e = cudaFuncSetAttribute(minv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                             p.K, scale, layout, (cx<float> *)minv);
+                                                             p.K, scale, layout, p.k_lo, (cx<float> *)minv);
     } else {
         e = cudaFuncSetAttribute(minv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                              p.K, scale, layout, (cx<double> *)minv);
+                                                              p.K, scale, layout, p.k_lo, (cx<double> *)minv);
     }
     count_launches(1);
     return cudaGetLastError();

@@ -38,11 +38,8 @@ using LD = LaneF64;
 constexpr int kTeams = 3;
 constexpr int kTeamThreads = 128;
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane
-constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B: exchange / transposes / mirror rows / E_theta
-constexpr int kEStride = 260;                         // E buffer: slot = (k' & 3) * 260 + (k' >> 2), conflict-free both ways
-constexpr int kEPlane = 4 * kEStride;                 // doubles per plane
-constexpr int kRegionY = 2 * kEPlane * 8;             // 16 640 B: E_phi (re plane, im plane)
-constexpr int kTeamBytes = kRegionX + kRegionY;
+constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B per team: exchange buffer / transpose planes / mirror rows
+constexpr int kTeamBytes = kRegionX;
 constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_4096^t, t < 1024)
 constexpr int kCtlF64 = 512;
 
@@ -51,7 +48,7 @@ struct T4kParams {
     double *efield;
     double *amp;
     int32_t *idx;
-    const double2 *minv;   // [n_events][K][4] complex (MINV_ROWS), scaled by 1/N
+    const double2 *minv;   // [n_events] MINV_Q4 planes [q][entry][C] complex, scaled by 1/N
     const double2 *tw1024; // W_1024^m
     const double2 *twN;    // W_4096^m
     long n_units;
@@ -88,15 +85,25 @@ __device__ __forceinline__ double2 w4096(const double2 *TQ, int t)
     return r;
 }
 
-// y[k1] *= W_1024^(k1 * lane); "P" plays the real part.
+// y[k1] *= W_1024^(k1 * lane); "P" plays the real part. The 31 twiddles of a lane are a geometric
+// sequence: two interleaved recurrences (even and odd k1, ratio W^{2 lane}) from TWO table reads
+// instead of 31. The shared-memory pipe, not the FP64 pipe, limits this kernel; 15 complex
+// multiplications per chain cost < 4e-15 of relative accuracy.
 __device__ __forceinline__ void pass_twiddle_d(double (&P)[32], double (&Q)[32], const double2 *__restrict__ T, int lane)
 {
+    const double2 w1 = T[32 + lane], w2 = T[64 + lane];     // W^{lane}, W^{2 lane}
+    double er = w2.x, ei = w2.y, orr = w1.x, oi = w1.y;      // current even / odd twiddle
     static_for<1, 32>([&](auto kc) {
         constexpr int k1 = decltype(kc)::value;
-        const double2 w = T[k1 * 32 + lane];
-        double a = P[k1] * w.x; a = fma(Q[k1], -w.y, a);
-        double b = P[k1] * w.y; b = fma(Q[k1], w.x, b);
+        const double wr = (k1 & 1) ? orr : er, wi = (k1 & 1) ? oi : ei;
+        double a = P[k1] * wr; a = fma(Q[k1], -wi, a);
+        double b = P[k1] * wi; b = fma(Q[k1], wr, b);
         P[k1] = a; Q[k1] = b;
+        if constexpr (k1 + 2 < 32) {                         // advance the chain just used by W^{2 lane}
+            double nr = wr * w2.x; nr = fma(-wi, w2.y, nr);
+            double ni = wr * w2.y; ni = fma(wi, w2.x, ni);
+            if (k1 & 1) { orr = nr; oi = ni; } else { er = nr; ei = ni; }
+        }
     });
 }
 __device__ __forceinline__ void transpose_plane_d(double (&P)[32], double *X, int lane)
@@ -150,7 +157,6 @@ unfold_t4k_f64_kernel(T4kParams p)
     int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + kTeams * 32) + team * 4;
     unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kTeamBytes;
     double *RX = reinterpret_cast<double *>(tb);            // region X
-    double *RY = reinterpret_cast<double *>(tb + kRegionX); // region Y
     double *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
 
     if (warp == 0) tmem_alloc_all(tmem_base);
@@ -162,7 +168,8 @@ unfold_t4k_f64_kernel(T4kParams p)
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
-    const uint32_t tenv = tmem_addr(*tmem_base, warp, team * 64);  // |z_theta|^2, 2 columns per row
+    const uint32_t tenv = tmem_addr(*tmem_base, warp, team * 128); // |z_theta|^2: 2 columns per sample, 64 columns
+    const uint32_t tephi = tenv + 64;                               // E_phi: 4 columns per band row
 
     const long u0 = p.n_units * (long)blockIdx.x / (long)gridDim.x;
     const long u1 = p.n_units * ((long)blockIdx.x + 1) / (long)gridDim.x;
@@ -172,7 +179,7 @@ unfold_t4k_f64_kernel(T4kParams p)
     for (long u = u0 + team; u < u1; u += kTeams) {
         const double *v = p.traces + (size_t)u * 2 * N;
         double *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
-        const double2 *M = p.minv + (size_t)(u / p.n_stations) * p.K * 4;
+        const double2 *M = p.minv + (size_t)(u / p.n_stations) * minv_q4_stride(p.k_lo, p.k_hi);
         if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(double));
 
         double P[32], Q[32];
@@ -191,7 +198,9 @@ unfold_t4k_f64_kernel(T4kParams p)
             const double y2r = ar - cr, y2i = ai - ci;
             const double y3r = br - di, y3i = bi + dr;           // b + i d
             const double2 w1 = TQ[m];                            // W_4096^m, m < 1024
-            const double2 w2 = w4096(TQ, 2 * m), w3 = w4096(TQ, 3 * m);
+            double2 w2, w3;                                      // W^{2m}, W^{3m} by multiplication: one table read, not three
+            w2.x = fma(w1.x, w1.x, -(w1.y * w1.y)); w2.y = (w1.x + w1.x) * w1.y;
+            w3.x = fma(w2.x, w1.x, -(w2.y * w1.y)); w3.y = fma(w2.x, w1.y, w2.y * w1.x);
             double t;
             t = y1r * w1.x; P[8 + jj] = fma(y1i, -w1.y, t); t = y1r * w1.y; Q[8 + jj] = fma(y1i, w1.x, t);
             t = y2r * w2.x; P[16 + jj] = fma(y2i, -w2.y, t); t = y2r * w2.y; Q[16 + jj] = fma(y2i, w2.x, t);
@@ -234,13 +243,15 @@ unfold_t4k_f64_kernel(T4kParams p)
             });
         }
         team_sync(team);
-        // ---- separation + a4 on the band rows: E stays in registers until every mirror read is done
-        double Etr[kRows], Eti[kRows], Epr[kRows], Epi[kRows];
+        // ---- separation + a4 on the band rows: E for this warp's bins k = 4 (lane + 32 r) + w, in registers
+        double Etr[kRows], Eti[kRows];
         {
             const double2 *PUB = reinterpret_cast<const double2 *>(RX);
             const int pw = (4 - w) & 3;
             const int plane = (w == 0) ? ((32 - lane) & 31) : (31 - lane);
             const int padd = (w == 0 && lane == 0) ? 1 : 0;      // q = 0, lane 0: mirror row 32 - r
+            const int C = (p.k_hi >> 2) - (p.k_lo >> 2) + 1;     // Minv columns per (q, entry) plane
+            const double2 *Mq = M + (size_t)w * 4 * C;
             static_for<0, kRows>([&](auto rc) {
                 constexpr int i = decltype(rc)::value;
                 constexpr int r = RLO + i;
@@ -249,10 +260,10 @@ unfold_t4k_f64_kernel(T4kParams p)
                 int prow = 31 - r + padd;
                 prow = prow > kMirHi ? kMirHi : prow;
                 const double2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
-                int j = k - p.k_lo;
-                j = j < 0 ? 0 : (j > p.K - 1 ? p.K - 1 : j);
-                const double2 m0 = ld_nc_d2(M + 4 * j), m1 = ld_nc_d2(M + 4 * j + 1);
-                const double2 m2 = ld_nc_d2(M + 4 * j + 2), m3 = ld_nc_d2(M + 4 * j + 3);
+                int c = lane + 32 * r - (p.k_lo >> 2);
+                c = c < 0 ? 0 : (c > C - 1 ? C - 1 : c);
+                const double2 m0 = ld_nc_d2(Mq + c), m1 = ld_nc_d2(Mq + C + c);
+                const double2 m2 = ld_nc_d2(Mq + 2 * C + c), m3 = ld_nc_d2(Mq + 3 * C + c);
                 const double v0r = P[r] + gm.x, v0i = Q[r] - gm.y;   // 2 V_0
                 const double v1r = Q[r] + gm.y, v1i = gm.x - P[r];   // 2 V_1
                 double er = m0.x * v0r; er = fma(-m0.y, v0i, er); er = fma(m1.x, v1r, er); er = fma(-m1.y, v1i, er);
@@ -260,57 +271,111 @@ unfold_t4k_f64_kernel(T4kParams p)
                 double fr = m2.x * v0r; fr = fma(-m2.y, v0i, fr); fr = fma(m3.x, v1r, fr); fr = fma(-m3.y, v1i, fr);
                 double fi = m2.x * v0i; fi = fma(m2.y, v0r, fi); fi = fma(m3.x, v1i, fi); fi = fma(m3.y, v1r, fi);
                 Etr[i] = inband ? er : 0.0; Eti[i] = inband ? ei : 0.0;
-                Epr[i] = inband ? fr : 0.0; Epi[i] = inband ? fi : 0.0;
+                // E_phi waits in tensor memory while the registers hold the theta transform
+                tmem_st64(tephi + 4 * i, (unsigned long long)__double_as_longlong(inband ? fr : 0.0));
+                tmem_st64(tephi + 4 * i + 2, (unsigned long long)__double_as_longlong(inband ? fi : 0.0));
             });
         }
-        team_sync(team);                                         // mirror rows consumed: region X becomes E_theta
-        {
-            // residue slot of bin k = 4 (lane + 32 r) + q: q * 260 + lane + 32 (r & 7); rows r and r + 8
-            // share a slot and at most one of them is in band (K <= 1024); unused slots are zeroed.
-            double *ETr = RX, *ETi = RX + kEPlane, *EPr = RY, *EPi = RY + kEPlane;
-            static_for<0, 8>([&](auto cc) {
-                constexpr int c8 = decltype(cc)::value;
-                constexpr int r1 = RLO + ((c8 - RLO) & 7);       // first band row with r & 7 == c8
-                double a = 0.0, b = 0.0, c = 0.0, d = 0.0;
-                if constexpr (r1 <= RHI) { a = Etr[r1 - RLO]; b = Eti[r1 - RLO]; c = Epr[r1 - RLO]; d = Epi[r1 - RLO]; }
-                if constexpr (r1 + 8 <= RHI) { a += Etr[r1 + 8 - RLO]; b += Eti[r1 + 8 - RLO]; c += Epr[r1 + 8 - RLO]; d += Epi[r1 + 8 - RLO]; }
-                const int slot = w * kEStride + lane + 32 * c8;
-                ETr[slot] = a; ETi[slot] = b; EPr[slot] = c; EPi[slot] = d;
-            });
-        }
-        team_sync(team);
+        team_sync(team);                                         // mirror rows consumed: region X is free for transposes
 
-        // ---- a5/a6: warp s = w produces samples n = 4 m + s; theta first, then phi
-        double best = -1.0; int bb = 0;
-        const int rslot = (lane & 3) * kEStride + (lane >> 2);
+        // ---- a5/a6: per polarisation, mirror image of the forward path. Warp q inverse-transforms its own
+        // bins Z[4 k' + q] (zero outside the band rows), multiplies by W_4096^{-m q}, the team exchanges,
+        // and the radix-4 step gives z[m + 1024 s], s = 0..3, for this thread's 8 values of m:
+        // contiguous 8-byte stores, 256 bytes per warp instruction.
+        double best = -1.0; int bn = 0;
 #pragma unroll 1
         for (int pol = 0; pol < 2; ++pol) {
-            const double *Er = pol ? RY : RX, *Ei = Er + kEPlane;
-            static_for<0, 32>([&](auto jc) {
-                constexpr int j = decltype(jc)::value;
-                P[brev5(j)] = Er[rslot + 8 * j];
-                Q[brev5(j)] = Ei[rslot + 8 * j];
-            });
-            if (w != 0) {                                        // E[k] W_4096^{-s k}, k = the band bin of residue k'
-                static_for<0, 32>([&](auto jc) {
-                    constexpr int j = decltype(jc)::value;
-                    const int kp = lane + 32 * j;
-                    const int k = kp + (((p.k_lo - kp + 1023) >> 10) << 10);
-                    const double2 tw = w4096(TQ, (w * k) & 4095);
-                    const double er = P[brev5(j)], ei = Q[brev5(j)];
-                    double a = er * tw.x; a = fma(ei, tw.y, a);
-                    double b = ei * tw.x; b = fma(er, -tw.y, b);
-                    P[brev5(j)] = a; Q[brev5(j)] = b;
+            if (pol == 0) {
+                static_for<0, 32>([&](auto kc) {
+                    constexpr int r = decltype(kc)::value;
+                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = 0.0; Q[brev5(r)] = 0.0; }
+                    else { P[brev5(r)] = Etr[r - RLO]; Q[brev5(r)] = Eti[r - RLO]; }
+                });
+            } else {
+                unsigned long long ev[2 * kRows];
+                static_for<0, kRows>([&](auto rc) {
+                    constexpr int i = decltype(rc)::value;
+                    ev[2 * i] = tmem_ld64(tephi + 4 * i);
+                    ev[2 * i + 1] = tmem_ld64(tephi + 4 * i + 2);
+                });
+                tmem_wait_ld();
+                static_for<0, kRows>([&](auto rc) {
+                    constexpr int i = decltype(rc)::value;
+                    tmem_ld_dep(ev[2 * i], ev[2 * i + 1]);
+                });
+                static_for<0, 32>([&](auto kc) {
+                    constexpr int r = decltype(kc)::value;
+                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = 0.0; Q[brev5(r)] = 0.0; }
+                    else {
+                        P[brev5(r)] = __longlong_as_double((long long)ev[2 * (r - RLO)]);
+                        Q[brev5(r)] = __longlong_as_double((long long)ev[2 * (r - RLO) + 1]);
+                    }
                 });
             }
-            if (pol == 0) team_sync(team);                       // everyone has E_theta before transposes reuse region X
-            fft1024_d(Q, P, XW, T, lane);                        // inverse: roles swapped
-            if (pol == 0) {
+            fft1024_d(Q, P, XW, T, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
+            if (w != 0) {
+                // u_q[m] conj(W_4096^{q m}), m = lane + 32 b: two interleaved recurrences over b (ratio W^{64 q})
+                const double2 r2 = w4096(TQ, 64 * w);
+                const double2 c0 = w4096(TQ, (w * lane) & 4095), c1 = w4096(TQ, (w * (lane + 32)) & 4095);
+                double er = c0.x, ei = c0.y, orr = c1.x, oi = c1.y;
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
-                    if (HAS_EF) ef[4 * (lane + 32 * b) + w] = P[b];
-                    double e2 = P[b] * P[b]; e2 = fma(Q[b], Q[b], e2);
-                    tmem_st64(tenv + 2 * b, (unsigned long long)__double_as_longlong(e2));
+                    const double wr = (b & 1) ? orr : er, wi = (b & 1) ? oi : ei;
+                    const double ur = P[b], ui = Q[b];
+                    double a = ur * wr; a = fma(ui, wi, a);
+                    double c = ui * wr; c = fma(ur, -wi, c);
+                    P[b] = a; Q[b] = c;
+                    if constexpr (b + 2 < 32) {
+                        double nr = wr * r2.x; nr = fma(-wi, r2.y, nr);
+                        double ni = wr * r2.y; ni = fma(wi, r2.x, ni);
+                        if (b & 1) { orr = nr; oi = ni; } else { er = nr; ei = ni; }
+                    }
+                });
+            }
+            team_sync(team);                                     // all transposes done: region X is the exchange buffer
+            {
+                double *XB = RX;                                 // [q][b][lane]
+                static_for<0, 32>([&](auto bc) {
+                    constexpr int b = decltype(bc)::value;
+                    XB[(w * 32 + b) * 32 + lane] = P[b];
+                });
+                team_sync(team);
+                static_for<0, 32>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;       // i = 8 q + jj
+                    P[i] = XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane];
+                });
+                team_sync(team);
+                static_for<0, 32>([&](auto bc) {
+                    constexpr int b = decltype(bc)::value;
+                    XB[(w * 32 + b) * 32 + lane] = Q[b];
+                });
+                team_sync(team);
+                static_for<0, 32>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    Q[i] = XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane];
+                });
+                team_sync(team);
+            }
+            // radix-4 step (inverse sign): z_s = sum_q (+i)^{s q} u_q, left in place at [8 s + jj]
+            static_for<0, 8>([&](auto jc) {
+                constexpr int jj = decltype(jc)::value;
+                const double ar = P[jj] + P[16 + jj], ai = Q[jj] + Q[16 + jj];
+                const double br = P[jj] - P[16 + jj], bi = Q[jj] - Q[16 + jj];
+                const double cr = P[8 + jj] + P[24 + jj], ci = Q[8 + jj] + Q[24 + jj];
+                const double dr = P[8 + jj] - P[24 + jj], di = Q[8 + jj] - Q[24 + jj];
+                P[jj] = ar + cr; Q[jj] = ai + ci;
+                P[8 + jj] = br - di; Q[8 + jj] = bi + dr;        // b + i d
+                P[16 + jj] = ar - cr; Q[16 + jj] = ai - ci;
+                P[24 + jj] = br + di; Q[24 + jj] = bi - dr;      // b - i d
+            });
+            // outputs: index i = 8 s + jj is sample n = lane + 32 (8 w + jj) + 1024 s (ascending in i)
+            const int nbase = lane + 256 * w;
+            if (pol == 0) {
+                static_for<0, 32>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    if (HAS_EF) ef[nbase + 32 * (i & 7) + 1024 * (i >> 3)] = P[i];
+                    double e2 = P[i] * P[i]; e2 = fma(Q[i], Q[i], e2);
+                    tmem_st64(tenv + 2 * i, (unsigned long long)__double_as_longlong(e2));
                 });
                 tmem_wait_st();
             } else {
@@ -328,17 +393,18 @@ unfold_t4k_f64_kernel(T4kParams p)
                     });
                     static_for<0, 8>([&](auto jc) {
                         constexpr int j = decltype(jc)::value;
-                        constexpr int b = 8 * c + j;
-                        if (HAS_EF) ef[N + 4 * (lane + 32 * b) + w] = P[b];
-                        double e2 = fma(P[b], P[b], __longlong_as_double((long long)ev[j]));
-                        e2 = fma(Q[b], Q[b], e2);
-                        if (e2 > best) { best = e2; bb = b; }
+                        constexpr int i = 8 * c + j;
+                        const int n = nbase + 32 * (i & 7) + 1024 * (i >> 3);
+                        if (HAS_EF) ef[N + n] = P[i];
+                        double e2 = fma(P[i], P[i], __longlong_as_double((long long)ev[j]));
+                        e2 = fma(Q[i], Q[i], e2);
+                        if (e2 > best) { best = e2; bn = n; }
                     });
                 });
             }
         }
         // ---- a6: lane -> warp -> team argmax, lowest index on ties in every stage
-        int bi = 4 * (lane + 32 * bb) + w;
+        int bi = bn;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             const double ob = __shfl_xor_sync(0xffffffffu, best, o);
