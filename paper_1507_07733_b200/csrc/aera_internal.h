@@ -51,7 +51,9 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
 //   MINV_Q4     : per direction 16 planes [q = k & 3][entry 0..3 as in MINV_ROWS][C] complex, column
 //                 (k >> 2) - (k_lo >> 2), C = (k_hi >> 2) - (k_lo >> 2) + 1; slots of bins outside the
 //                 band are never written or used                                       (team kernel)
-enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2 };
+//   MINV_Q32    : per direction 64 float4 planes [q = k & 31][A | B as in MINV_PACKED][C], column
+//                 (k >> 5) - (k_lo >> 5), C = (k_hi >> 5) - (k_lo >> 5) + 1              (long-trace kernel)
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3 };
 // complex elements per direction in the MINV_Q4 layout (<= 4 K + 32)
 __host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
@@ -77,6 +79,12 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
 bool t4k_f64_supported(int dtype, const PlanDev &p);
 cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                   void *amp, int32_t *idx, const void *minv, cudaStream_t s);
+
+// ---- unfold_long_f32.cu: multi-pass kernel for N = 65536 fp32 through an L2-resident scratch (configs[4])
+bool long_f32_supported(int dtype, const PlanDev &p);
+size_t long_f32_scratch_bytes(const PlanDev &p);
+cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+                                   void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s);
 
 // ---- scan_w32.cu: direction scan for N = 2048 fp32, band rows 10..28 (configs[2])
 bool scan_w32_supported(int dtype, const PlanDev &p);

@@ -234,13 +234,21 @@ struct WsLayout {
 };
 
 // Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
-WsLayout ws_layout(aera_op_t op, int dtype, int N, int K, long n_dirs, int n_stations)
+WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs, int n_stations)
 {
+    const int k_hi = k_lo + K - 1;
+    PlanDev band{}; band.N = N; band.k_lo = k_lo; band.k_hi = k_hi; band.K = K;
     WsLayout w{};
     const size_t cb = cplx_bytes(dtype);
     size_t o = 0;
-    w.off_minv = o; o = align_up(o + (size_t)n_dirs * (K * 4 + 32) * cb); // + 32: MINV_Q4 plane padding
-    w.off_scratch = o; o = align_up(o + generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations));
+    size_t per_dir = (size_t)K * 4 + 32;                                  // + 32: MINV_Q4 plane padding
+    const size_t q32 = (size_t)128 * ((k_hi >> 5) - (k_lo >> 5) + 1);     // MINV_Q32 planes
+    if (q32 > per_dir) per_dir = q32;
+    w.off_minv = o; o = align_up(o + (size_t)n_dirs * per_dir * cb);
+    size_t scratch = generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations);
+    if (op == AERA_OP_UNFOLD && long_f32_supported(dtype, band) && long_f32_scratch_bytes(band) > scratch)
+        scratch = long_f32_scratch_bytes(band);
+    w.off_scratch = o; o = align_up(o + scratch);
     w.off_spectra = o;
     if (op == AERA_OP_SCAN) { // room for either scan path's station spectra
         size_t a = generic_scan_spectra_bytes(dtype, K, n_stations), b = scan_w32_spectra_bytes(n_stations);
@@ -372,7 +380,7 @@ size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dty
     if (n_events_or_dirs < 0) { fail(AERA_ERR_INVALID_ARG, "negative count"); return 0; }
     int k_lo, k_hi;
     if (compute_band(pattern->desc, n_samples, fs_hz, &k_lo, &k_hi) != AERA_OK) return 0;
-    return ws_layout(op, dtype, n_samples, k_hi - k_lo + 1, n_events_or_dirs, n_stations).total;
+    return ws_layout(op, dtype, n_samples, k_lo, k_hi - k_lo + 1, n_events_or_dirs, n_stations).total;
 }
 
 aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
@@ -392,22 +400,26 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
     Plan *pl = nullptr;
     st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
     if (st != AERA_OK) return st;
-    const WsLayout w = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.K, n_events, n_stations);
+    const WsLayout w = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, n_events, n_stations);
     if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
 
     const bool warp_path = kernel_variant() == 0 && w32_supported(dtype, pl->dev);
     const bool team_path = kernel_variant() == 0 && t4k_f64_supported(dtype, pl->dev);
+    const bool long_path = kernel_variant() == 0 && long_f32_supported(dtype, pl->dev);
     // the warp and team kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
-                                warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : MINV_ROWS),
-                                ((warp_path || team_path) ? 1.0 : 2.0) / (double)n_samples, s);
+                                warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS)),
+                                ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
     else if (team_path)
         e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
+    else if (long_path)
+        e = launch_unfold_long_f32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv,
+                                   ws + w.off_scratch, s);
     else
         e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
                                   ws + w.off_minv, ws + w.off_scratch, s);
@@ -433,7 +445,7 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
     Plan *pl = nullptr;
     st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
     if (st != AERA_OK) return st;
-    const WsLayout w = ws_layout(AERA_OP_SCAN, dtype, n_samples, pl->dev.K, n_dirs, n_stations);
+    const WsLayout w = ws_layout(AERA_OP_SCAN, dtype, n_samples, pl->dev.k_lo, pl->dev.K, n_dirs, n_stations);
     if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
@@ -487,7 +499,7 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
     if (st != AERA_OK) return st;
     const size_t need_trace = (size_t)chunk_events * event_bytes;
     const size_t need_units = (size_t)chunk_events * n_stations;
-    const size_t need_ws = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.K, chunk_events, n_stations).total;
+    const size_t need_ws = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, chunk_events, n_stations).total;
     if (need_trace > hp.cap_trace_bytes || need_units > hp.cap_units || need_ws > hp.cap_ws || (size_t)chunk_events > hp.cap_events) {
         cudaDeviceSynchronize();
         for (int i = 0; i < 2; ++i) {

@@ -156,6 +156,12 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
             const int k = k_lo + j, C = ((k_lo + K - 1) >> 2) - (k_lo >> 2) + 1;
             cx<T> *q = minv + (size_t)d * 16 * C + (size_t)(k & 3) * 4 * C + ((k >> 2) - (k_lo >> 2));
             q[0] = mt0; q[C] = mt1; q[2 * C] = mp0; q[3 * C] = mp1;
+        } else if (layout == MINV_Q32) {
+            const int k = k_lo + j, C = ((k_lo + K - 1) >> 5) - (k_lo >> 5) + 1;
+            cx<T> *a = minv + (size_t)d * 128 * C + ((size_t)(k & 31) * 2 * C + ((k >> 5) - (k_lo >> 5))) * 2;
+            cx<T> *b = a + (size_t)C * 2;
+            a[0].re = mt0.re; a[0].im = mp0.re; a[1].re = mt0.im; a[1].im = mp0.im;
+            b[0].re = mt1.re; b[0].im = mp1.re; b[1].re = mt1.im; b[1].im = mp1.im;
         } else { // MINV_PACKED: two planes per direction, (theta, phi) side by side so a packed
                  // f32x2 load yields both: A[j] = {t0.re, p0.re, t0.im, p0.im}, B[j] = {t1.re, p1.re, t1.im, p1.im}
             cx<T> *a = minv + (size_t)d * K * 4 + (size_t)j * 2, *b = a + (size_t)K * 2;
