@@ -33,7 +33,9 @@ namespace aera {
 namespace {
 
 constexpr int kLN = 65536;
-constexpr int kLWarps = 12;
+constexpr int kLWarps = 8;                 // warps per CTA
+constexpr int kLCluster = 2;               // CTAs per station (thread-block cluster): 16 warps, every phase is 2 balanced rounds
+constexpr int kLTeam = kLWarps * kLCluster;
 constexpr size_t kYBytes = (size_t)32 * 1024 * 16;            // Y[q][mm] two 8-byte planes; reused as U[2][16][1024]
 // band geometry of the one instantiation (configs[4]: k = 1311 .. 13107)
 constexpr int kP2Lo = 1, kP2Hi = 12;      // phase 2 rows (k' >> 5, k' = k >> 5)
@@ -55,15 +57,42 @@ struct LongParams {
     int k_lo, k_hi, K, C;  // C = (k_hi >> 5) - (k_lo >> 5) + 1
 };
 
-__device__ __forceinline__ R ld_cg_b64(const void *p) // L2-only: scratch written by other warps of this CTA
+// L2 residency: the scratch (148 x 704 KB) must stay in the 126 MB L2 while 1 MB per station streams
+// through it, so scratch accesses carry an evict_last policy and the streamed traces / E-field an
+// evict_first policy (createpolicy + .L2::cache_hint).
+__device__ __forceinline__ unsigned long long policy_evict_last()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ unsigned long long policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// scratch: L2-only loads (written by other warps of this CTA), evict_last
+__device__ __forceinline__ R ld_sc(const void *p, unsigned long long pol)
 {
     R r;
-    asm volatile("ld.global.cg.b64 %0, [%1];" : "=l"(r.v) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(r.v) : "l"(p), "l"(pol) : "memory");
     return r;
 }
-__device__ __forceinline__ void st_cg_b64(void *p, R v)
+__device__ __forceinline__ void st_sc(void *p, R v, unsigned long long pol)
 {
-    asm volatile("st.global.cg.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
+    asm volatile("st.global.cg.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(p), "l"(v.v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ R ld_stream_pol(const void *p, unsigned long long pol)
+{
+    R r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(r.v) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ void st_stream_f4(void *p, float4 v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;"
+                 ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
 }
 
 // W_65536^x from two 256-entry tables: W^x = TA[x >> 8] TB[x & 255] (one complex multiplication in fp32).
@@ -97,6 +126,24 @@ __device__ __forceinline__ void fft1024_loop(R (&A)[32], R (&B)[32], R *X, const
         second = 1;
         asm volatile("" : "+r"(second));
     }
+}
+// all threads of the cluster; orders global-memory accesses between the two CTAs (release / acquire)
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ unsigned cluster_rank()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ float2 cmulf(float2 a, float2 b)
+{
+    float2 r;
+    r.x = fmaf(a.x, b.x, -(a.y * b.y));
+    r.y = fmaf(a.x, b.y, a.y * b.x);
+    return r;
 }
 __device__ __forceinline__ void pair_sync(int pair)
 {
@@ -137,7 +184,7 @@ __device__ __forceinline__ void ifft16(R (&xr)[16], R (&xi)[16])
 }
 
 template <bool HAS_EF>
-__global__ void __launch_bounds__(kLWarps * 32, 1)
+__global__ void __cluster_dims__(kLCluster, 1, 1) __launch_bounds__(kLWarps * 32, 1)
 unfold_long_f32_kernel(LongParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -147,6 +194,9 @@ unfold_long_f32_kernel(LongParams p)
     unsigned long long *peak = reinterpret_cast<unsigned long long *>(TB + 256);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
+    const int crank = (int)cluster_rank();
+    const int gw = crank * kLWarps + warp;                              // warp index within the station's team of 16
+    const long cluster_id = blockIdx.x / kLCluster, n_clusters = gridDim.x / kLCluster;
     R *X = reinterpret_cast<R *>(smem + 8192 + 4096 + 128 + (size_t)warp * kXBytes);   // transpose plane / mirror rows
     R *Xpartner = reinterpret_cast<R *>(smem + 8192 + 4096 + 128 + (size_t)(warp ^ 1) * kXBytes);
 
@@ -161,50 +211,57 @@ unfold_long_f32_kernel(LongParams p)
     if (threadIdx.x == 0) *peak = 0ull;
     __syncthreads();
 
-    unsigned char *sc = p.scratch + (size_t)blockIdx.x * p.scratch_stride;
+    unsigned char *sc = p.scratch + (size_t)cluster_id * p.scratch_stride;
+    unsigned long long *gpeak = reinterpret_cast<unsigned long long *>(sc + p.scratch_stride - 64);  // [2] per-CTA peaks
     R *YA = reinterpret_cast<R *>(sc), *YB = YA + 32 * 1024;
     R *EA = reinterpret_cast<R *>(sc + kYBytes), *EB = EA + 32 * p.C;
+    R *H0 = EB + 32 * p.C;                                              // [pol 2][t 16][mm 1024] parked (s = 0, 1) pairs
     const int C = p.C, c_lo = p.k_lo >> 5;
+    const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
 
 #pragma unroll 1
-    for (long u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+    for (long u = cluster_id; u < p.n_units; u += n_clusters) {
         const float *v0 = p.traces + (size_t)u * 2 * kLN, *v1 = v0 + kLN;
         float *ef = HAS_EF ? p.efield + (size_t)u * 2 * kLN : nullptr;
         const float4 *Mev = p.minv + (size_t)(u / p.n_stations) * 64 * C;
 
         // ---------------- phase 1: loads + 32-point transform over j' + twiddle -> Y
 #pragma unroll 1
-        for (int mb = warp; mb < 32; mb += kLWarps) {
+        for (int mb = gw; mb < 32; mb += kLTeam) {
             const int mm = lane + 32 * mb;
             R A[32], B[32];
             static_for<0, 32>([&](auto jc) {
                 constexpr int j = decltype(jc)::value;
-                A[brev5(j)] = ld_stream_b64(v0 + 2 * (mm + 1024 * j));
-                B[brev5(j)] = ld_stream_b64(v1 + 2 * (mm + 1024 * j));
+                A[brev5(j)] = ld_stream_pol(v0 + 2 * (mm + 1024 * j), pol_first);
+                B[brev5(j)] = ld_stream_pol(v1 + 2 * (mm + 1024 * j), pol_first);
             });
             fft32<L>(A, B);
+            // W_32768^{q mm} = W_N^{2 q mm}: geometric in q; recurrences of 8 steps re-seeded from the table
+            const float2 rat = w64k(TA, TB, (unsigned)(2 * mm));
+            float2 w = rat;
             static_for<0, 32>([&](auto qc) {
                 constexpr int q = decltype(qc)::value;
                 if constexpr (q > 0) {
-                    const float2 w = w64k(TA, TB, (unsigned)(2 * q * mm));
+                    if constexpr ((q & 7) == 0) w = w64k(TA, TB, (unsigned)(2 * q * mm));
                     cmul_packed(A[q], B[q], w.x, w.y);
+                    if constexpr ((q & 7) != 7) w = cmulf(w, rat);
                 }
-                st_cg_b64(YA + q * 1024 + mm, A[q]);
-                st_cg_b64(YB + q * 1024 + mm, B[q]);
+                st_sc(YA + q * 1024 + mm, A[q], pol_last);
+                st_sc(YB + q * 1024 + mm, B[q], pol_last);
             });
         }
-        __syncthreads();
+        cluster_sync_all();
 
         // ---------------- phase 2: 1024-point transform per q, separation with the pair partner, fold, a4 -> E
 #pragma unroll 1
-        for (int pt = warp >> 1; pt < 16; pt += kLWarps / 2) {
+        for (int pt = gw >> 1; pt < 16; pt += kLTeam / 2) {
             const int role = warp & 1;
             const int q = pt == 0 ? 16 * role : (role ? 32 - pt : pt);
             R A[32], B[32];
             static_for<0, 32>([&](auto jc) {
                 constexpr int j = decltype(jc)::value;
-                A[brev5(j)] = ld_cg_b64(YA + q * 1024 + lane + 32 * j);
-                B[brev5(j)] = ld_cg_b64(YB + q * 1024 + lane + 32 * j);
+                A[brev5(j)] = ld_sc(YA + q * 1024 + lane + 32 * j, pol_last);
+                B[brev5(j)] = ld_sc(YB + q * 1024 + lane + 32 * j, pol_last);
             });
             fft1024_loop(A, B, X, T, lane);     // lane k1, register k2: G_r[32 (k1 + 32 k2) + q], r = 0,1 packed
             static_for<kMirLoL, 32>([&](auto rc) {
@@ -217,8 +274,12 @@ unfold_long_f32_kernel(LongParams p)
             const int plane = q == 0 ? ((32 - lane) & 31) : (31 - lane);
             const int padd = (q == 0 && lane == 0) ? 1 : 0;
             const float4 *MA = Mev + (size_t)(2 * q) * C, *MB = MA + C;
+            const float2 rat = TA[4];                                // W_N^{1024}: k grows by 1024 per row
+            float2 w = make_float2(1.f, 0.f);
             static_for<kP2Lo, kP2Hi + 1>([&](auto rc) {
                 constexpr int k2 = decltype(rc)::value;
+                if constexpr (((k2 - kP2Lo) % 6) == 0) w = w64k(TA, TB, (unsigned)(32 * (lane + 32 * k2) + q));   // W_N^k
+                else w = cmulf(w, rat);
                 const int kp = lane + 32 * k2, k = 32 * kp + q;
                 const bool inband = k >= p.k_lo && k <= p.k_hi;
                 const int prow = 31 - k2 + padd - kMirLoL;
@@ -228,7 +289,6 @@ unfold_long_f32_kernel(LongParams p)
                 float f0r0, f0r1, f0i0, f0i1, f1r0, f1r1, f1i0, f1i1;
                 L::unpack(f0r, f0r0, f0r1); L::unpack(f0i, f0i0, f0i1);
                 L::unpack(f1r, f1r0, f1r1); L::unpack(f1i, f1i0, f1i1);
-                const float2 w = w64k(TA, TB, (unsigned)k);          // W_N^k
                 float v0r = fmaf(w.x, f0r1, f0r0); v0r = fmaf(-w.y, f0i1, v0r);
                 float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
                 float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
@@ -242,11 +302,11 @@ unfold_long_f32_kernel(LongParams p)
                 R ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
                 ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
                 if (!inband) { er = L::zero(); ei = L::zero(); }
-                if (c >= 0 && c < C) { st_cg_b64(EA + q * C + c, er); st_cg_b64(EB + q * C + c, ei); }
+                if (c >= 0 && c < C) { st_sc(EA + q * C + c, er, pol_last); st_sc(EB + q * C + c, ei, pol_last); }
             });
             pair_sync(warp >> 1);                       // mirror rows consumed before the next transposes
         }
-        __syncthreads();
+        cluster_sync_all();
 
         R *UA = YA, *UB = YB;                           // U[sl][q'][mm] reuses Y (index (16 sl + q') * 1024 + mm)
         float best = -1.0f; int bn = 0;
@@ -254,10 +314,12 @@ unfold_long_f32_kernel(LongParams p)
         for (int h = 0; h < 2; ++h) {
             // ---------------- phase 3: task (s = 2h + sl, q'): pruned inverse 1024-point transform -> U
 #pragma unroll 1
-            for (int ti = warp; ti < 32; ti += kLWarps) {
+            for (int ti = gw; ti < 32; ti += kLTeam) {
                 const int sl = ti >> 4, qp = ti & 15, s = 2 * h + sl;
                 const int q = qp + 16 * (lane & 1);                 // bin k = 16 k'' + q' = 32 k' + q
                 R A[32], B[32];                                      // inverse roles: A = Im, B = Re
+                const float2 rin = w64k(TA, TB, (unsigned)(512 * s));     // k grows by 512 per row
+                float2 win = make_float2(1.f, 0.f);
                 static_for<0, 32>([&](auto jc) {
                     constexpr int j = decltype(jc)::value;
                     if constexpr (j < kP3Lo || j > kP3Hi) { A[brev5(j)] = L::zero(); B[brev5(j)] = L::zero(); }
@@ -265,30 +327,34 @@ unfold_long_f32_kernel(LongParams p)
                         const int kpp = lane + 32 * j;
                         const int c = (kpp >> 1) - c_lo;
                         R er = L::zero(), ei = L::zero();
-                        if (c >= 0 && c < C) { er = ld_cg_b64(EA + q * C + c); ei = ld_cg_b64(EB + q * C + c); }
-                        if (s != 0) {                                // E[k] conj(W_N^{s k})
-                            const float2 w = w64k(TA, TB, (unsigned)(s * (16 * kpp + qp)));
-                            cmul_packed(er, ei, w.x, -w.y);
+                        if (c >= 0 && c < C) { er = ld_sc(EA + q * C + c, pol_last); ei = ld_sc(EB + q * C + c, pol_last); }
+                        if (s != 0) {                                // E[k] conj(W_N^{s k}), recurrences of 8 rows
+                            if constexpr (((j - kP3Lo) & 7) == 0) win = w64k(TA, TB, (unsigned)(s * (16 * kpp + qp)));
+                            else win = cmulf(win, rin);
+                            cmul_packed(er, ei, win.x, -win.y);
                         }
                         B[brev5(j)] = er; A[brev5(j)] = ei;
                     }
                 });
                 fft1024_loop(A, B, X, T, lane);                      // lane a, register b: u[mm = a + 32 b] = B + i A
+                const float2 rout = w64k(TA, TB, (unsigned)(128 * qp)); // mm grows by 32 per register
+                float2 wout = make_float2(1.f, 0.f);
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
                     const int mm = lane + 32 * b;
                     if (qp != 0) {                                   // conj(W_16384^{mm q'}) = conj(W_N^{4 mm q'})
-                        const float2 w = w64k(TA, TB, (unsigned)(4 * qp * mm));
-                        cmul_packed(B[b], A[b], w.x, -w.y);
+                        if constexpr ((b & 7) == 0) wout = w64k(TA, TB, (unsigned)(4 * qp * mm));
+                        else wout = cmulf(wout, rout);
+                        cmul_packed(B[b], A[b], wout.x, -wout.y);
                     }
-                    st_cg_b64(UA + (16 * sl + qp) * 1024 + mm, B[b]);
-                    st_cg_b64(UB + (16 * sl + qp) * 1024 + mm, A[b]);
+                    st_sc(UA + (16 * sl + qp) * 1024 + mm, B[b], pol_last);
+                    st_sc(UB + (16 * sl + qp) * 1024 + mm, A[b], pol_last);
                 });
             }
-            __syncthreads();
+            cluster_sync_all();
             // ---------------- phase 4: task mb: 16-point inverse transforms over q' for s = 2h, 2h+1; outputs
 #pragma unroll 1
-            for (int mb = warp; mb < 32; mb += kLWarps) {
+            for (int mb = gw; mb < 32; mb += kLTeam) {
                 const int mm = lane + 32 * mb;
                 R re0[16];
                 static_for<0, 2>([&](auto sc_) {
@@ -296,8 +362,8 @@ unfold_long_f32_kernel(LongParams p)
                     R xr[16], xi[16];
                     static_for<0, 16>([&](auto qc) {
                         constexpr int qp = decltype(qc)::value;
-                        xr[qp] = ld_cg_b64(UA + (16 * sl + qp) * 1024 + mm);
-                        xi[qp] = ld_cg_b64(UB + (16 * sl + qp) * 1024 + mm);
+                        xr[qp] = ld_sc(UA + (16 * sl + qp) * 1024 + mm, pol_last);
+                        xi[qp] = ld_sc(UB + (16 * sl + qp) * 1024 + mm, pol_last);
                     });
                     ifft16(xr, xi);                                  // [4 c + d] holds t = c + 4 d
                     static_for<0, 16>([&](auto ic) {
@@ -310,15 +376,27 @@ unfold_long_f32_kernel(LongParams p)
                         if (e2 > best || (e2 == best && n < bn)) { best = e2; bn = n; }
                         if (sl == 0) re0[i] = xr[i];
                         else if (HAS_EF) {
+                            // Re z of the four sample phases of one 16-byte quad come from two passes (h = 0, 1):
+                            // pass 0 parks its (s = 0, 1) pairs in the L2-resident scratch, pass 1 stores whole
+                            // quads, so every 32-byte sector of the E-field is written once and in full.
                             float t0, p0, t1, p1;
                             L::unpack(re0[i], t0, p0); L::unpack(xr[i], t1, p1);
-                            st_global_b64(ef + (n - 1), L::pack(t0, t1));            // e_theta[n-1], e_theta[n]
-                            st_global_b64(ef + kLN + (n - 1), L::pack(p0, p1));      // e_phi
+                            R *hp = H0 + (size_t)t * 1024 + mm;
+                            if (h == 0) {
+                                st_sc(hp, L::pack(t0, t1), pol_last);
+                                st_sc(hp + 16 * 1024, L::pack(p0, p1), pol_last);
+                            } else {
+                                const R a = ld_sc(hp, pol_last), b = ld_sc(hp + 16 * 1024, pol_last);
+                                float a0, a1, b0, b1;
+                                L::unpack(a, a0, a1); L::unpack(b, b0, b1);
+                                st_stream_f4(ef + (n - 3), make_float4(a0, a1, t0, t1), pol_first);
+                                st_stream_f4(ef + kLN + (n - 3), make_float4(b0, b1, p0, p1), pol_first);
+                            }
                         }
                     });
                 });
             }
-            __syncthreads();
+            if (h == 0) cluster_sync_all();                          // U is rewritten by the next pair's phase 3
         }
         // ---------------- a6: lane -> warp -> CTA argmax (lowest index on ties: key = value bits, ~index)
 #pragma unroll
@@ -330,11 +408,21 @@ unfold_long_f32_kernel(LongParams p)
         if (lane == 0)
             atomicMax(peak, ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xffffffffu - (unsigned)bn));
         __syncthreads();
-        if (threadIdx.x == 0) {
-            const unsigned long long key = *peak;
+        if (threadIdx.x == 0) {                                      // this CTA's peak -> the cluster's slot
+            asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(gpeak + crank), "l"(*peak) : "memory");
+            *peak = 0ull;
+        }
+        cluster_sync_all();                                          // also: next station's phase 1 may overwrite Y / U
+        if (crank == 0 && threadIdx.x == 0) {
+            unsigned long long key = 0ull;
+#pragma unroll
+            for (int c = 0; c < kLCluster; ++c) {
+                unsigned long long kc;
+                asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(kc) : "l"(gpeak + c) : "memory");
+                key = kc > key ? kc : key;
+            }
             p.amp[u] = sqrtf(__uint_as_float((unsigned)(key >> 32)));
             p.idx[u] = (int)(0xffffffffu - (unsigned)(key & 0xffffffffu));
-            *peak = 0ull;
         }
     }
 }
@@ -351,9 +439,9 @@ bool long_f32_supported(int dtype, const PlanDev &p)
 static size_t long_stride(const PlanDev &p)
 {
     const size_t C = (size_t)((p.k_hi >> 5) - (p.k_lo >> 5) + 1);
-    return (kYBytes + 2 * 32 * C * 8 + 255) & ~(size_t)255;
+    return (kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | per-CTA peaks
 }
-size_t long_f32_scratch_bytes(const PlanDev &p) { return 148 * long_stride(p); }
+size_t long_f32_scratch_bytes(const PlanDev &p) { return (148 / kLCluster) * long_stride(p); }
 
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                    void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
@@ -368,7 +456,7 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.C = (p.k_hi >> 5) - (p.k_lo >> 5) + 1;
     const size_t smem = 8192 + 4096 + 128 + (size_t)kLWarps * kXBytes;
-    const long grid = n_units < 148 ? n_units : 148;
+    const long grid = kLCluster * (n_units < 148 / kLCluster ? n_units : 148 / kLCluster);
     cudaError_t e;
     if (efield) {
         e = cudaFuncSetAttribute(unfold_long_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
