@@ -238,3 +238,56 @@ def test_library_is_loaded_and_counts_launches(B):
     run_gpu_batch(B, wl, table_for(wl), tr, dirs)
     assert B.aera_launch_count() >= n0 + 3  # repack + minv + unfold
     assert B.LIBRARY_PATH.endswith("libaera_unfold.so")
+
+
+# ------------------------------------------------------------------ full sizes, bench.py's launch configuration
+def _full_size_case(B, orc, cfg, n_events, sample_units, n_canon):
+    """The whole batch of a config in ONE call, exactly as bench.py launches it (same input builder: a
+    canonical block of seeded events tiled to the batch); sampled units are checked one by one against the
+    oracle, every unit against properties that hold at any size (finite, index in range, tiled copies of the
+    same event give bit-identical results)."""
+    import bench
+    wl = ai.WORKLOADS[cfg]
+    H = table_for(wl)
+    dt = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    host_tr, host_dirs, _, _ = bench.build_inputs(wl, n_events, 0, pinned=False, n_canon=n_canon)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    try:
+        d_tr = host_tr.cuda()
+        ef, amp, idx = B.aera_unfold_batch(pat, d_tr, host_dirs.cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        amp_h = amp.cpu().numpy(); idx_h = idx.cpu().numpy()
+        assert np.isfinite(amp_h).all() and (amp_h > 0).all()
+        assert (idx_h >= 0).all() and (idx_h < wl.n_samples).all()
+        if n_events >= 2 * n_canon:     # event e and e + n_canon are the same input at different addresses
+            assert np.array_equal(amp_h[:n_canon], amp_h[n_canon:2 * n_canon])
+            assert np.array_equal(idx_h[:n_canon], idx_h[n_canon:2 * n_canon])
+            assert torch.equal(ef[0], ef[n_canon])
+        S = wl.n_stations
+        ev_ids = sorted({u // S for u in sample_units})
+        tr_s = np.stack([host_tr[u // S, u % S].numpy() for u in sample_units])
+        dirs_s = np.stack([host_dirs[u // S].numpy() for u in sample_units])
+        ref = orc.unfold_batch(wl.grid, H, wl.fs_hz, tr_s, dirs_s, want_env2=True)
+        ef_s = np.stack([ef[u // S, u % S].cpu().numpy() for u in sample_units])
+        rep = compare(wl.dtype, ef_s, np.array([amp_h[u // S, u % S] for u in sample_units]),
+                      np.array([idx_h[u // S, u % S] for u in sample_units]), ref)
+        print(f"\n[full-size cfg{cfg}: {n_events} events x {S} stations, {len(sample_units)} sampled units, events {ev_ids[:4]}..] {rep}")
+        assert rep.ok(TOL[wl.dtype]), str(rep)
+    finally:
+        pat.free()
+
+
+def test_full_size_config1(B, orc):
+    rng = np.random.default_rng(11)
+    units = sorted(set(rng.integers(0, 124000, size=60).tolist()) | {0, 123999, 837, 838})   # incl. a CTA boundary
+    _full_size_case(B, orc, 1, 1000, units, n_canon=200)
+
+
+def test_full_size_config3(B, orc):
+    rng = np.random.default_rng(13)
+    units = sorted(set(rng.integers(0, 2000 * 40, size=40).tolist()) | {0, 79999})
+    _full_size_case(B, orc, 3, 2000, units, n_canon=200)    # bench.py's default size for configs[3]
+
+
+def test_full_size_config4(B, orc):
+    _full_size_case(B, orc, 4, 100, [0, 5000, 12399], n_canon=100)
