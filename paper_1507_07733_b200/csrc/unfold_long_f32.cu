@@ -1,11 +1,13 @@
 // Long-trace fused unfolding kernel for N = 65536 fp32 (BASELINE configs[4]):
-// a multi-pass transform whose intermediates live in an L2-resident per-CTA scratch, one station per
-// CTA at a time (persistent, one CTA of 12 warps per SM), every warp-level piece shared with the
-// N = 2048 kernel (w32_common.cuh: 32-point register FFTs, 1024-point warp FFTs, packed f32x2 lanes).
+// a multi-pass transform whose intermediates live in an L2-resident per-station scratch. One station per
+// thread-block CLUSTER of 8 CTAs x 4 warps (32 warps: every phase below is one round of 32 warp tasks),
+// three CTAs of three different stations per SM (12 warps whose phases are decoupled), persistent;
+// every warp-level piece is shared with the N = 2048 kernel (w32_common.cuh: 32-point register FFTs,
+// 1024-point warp FFTs, packed f32x2 lanes).
 //
 // One station's complex buffer (512 KB) is beyond an SM's shared memory (227 KB) and distributed
 // shared memory is slower than L2 on this part (~21 B/clk/SM against ~43 B/clk/SM of L2), so the
-// passes exchange through global memory that stays in the 126 MB L2: 148 CTAs x 704 KB.
+// passes exchange through global memory that stays in the 126 MB L2: <= 55 clusters x 0.96 MB.
 //
 //   phase 1 (32 warp tasks)  a1 + first forward pass. g_r[m] = v0[2m+r] + i v1[2m+r], r = 0,1 in the two
 //       packed halves (an 8-byte load of channel 0 IS the packed real part), m = mm + 1024 j'. Task mb:
@@ -25,16 +27,20 @@
 //       8-byte (s = 2h, 2h+1) pairs, env^2 = |z_theta|^2 + |z_phi|^2 running argmax, then a 64-bit
 //       shared-memory atomicMax of (env^2 bits, ~index) across the CTA's tasks.
 //
-// HBM traffic per station: 512 KB read once, 512 KB + 8 B written once (as two half-sector passes,
-// see DESIGN.md). L2 traffic per station: ~5 MB (the real roofline of this kernel, with the FP32 pipe).
+// HBM traffic per station: 512 KB read once, 512 KB + 8 B written once (the first pair's Re z is parked
+// in the scratch so that the second pass stores whole 16-byte quads). L2 traffic per station: ~5 MB (the real roofline of this kernel, with the FP32 pipe).
+#include <cstdio>
+#include <cstdlib>
 #include "w32_common.cuh"
 
 namespace aera {
 namespace {
 
 constexpr int kLN = 65536;
-constexpr int kLWarps = 8;                 // warps per CTA
-constexpr int kLCluster = 2;               // CTAs per station (thread-block cluster): 16 warps, every phase is 2 balanced rounds
+constexpr int kLWarps = 4;                 // warps per CTA
+constexpr int kLCtasPerSm = 3;             // 12 warps per SM, from three different stations (phases decoupled)
+constexpr int kLCluster = 8;               // CTAs per station (thread-block cluster): 32 warps, every phase (32 tasks) is ONE round
+constexpr int kLMaxClusters = 148 * kLCtasPerSm / kLCluster;   // 55 stations in flight
 constexpr int kLTeam = kLWarps * kLCluster;
 constexpr size_t kYBytes = (size_t)32 * 1024 * 16;            // Y[q][mm] two 8-byte planes; reused as U[2][16][1024]
 // band geometry of the one instantiation (configs[4]: k = 1311 .. 13107)
@@ -57,7 +63,7 @@ struct LongParams {
     int k_lo, k_hi, K, C;  // C = (k_hi >> 5) - (k_lo >> 5) + 1
 };
 
-// L2 residency: the scratch (148 x 704 KB) must stay in the 126 MB L2 while 1 MB per station streams
+// L2 residency: the scratch (<= 55 x 0.96 MB) must stay in the 126 MB L2 while 1 MB per station streams
 // through it, so scratch accesses carry an evict_last policy and the streamed traces / E-field an
 // evict_first policy (createpolicy + .L2::cache_hint).
 __device__ __forceinline__ unsigned long long policy_evict_last()
@@ -127,7 +133,7 @@ __device__ __forceinline__ void fft1024_loop(R (&A)[32], R (&B)[32], R *X, const
         asm volatile("" : "+r"(second));
     }
 }
-// all threads of the cluster; orders global-memory accesses between the two CTAs (release / acquire)
+// all threads of the cluster; orders global-memory accesses between its CTAs (release / acquire)
 __device__ __forceinline__ void cluster_sync_all()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -184,7 +190,7 @@ __device__ __forceinline__ void ifft16(R (&xr)[16], R (&xi)[16])
 }
 
 template <bool HAS_EF>
-__global__ void __cluster_dims__(kLCluster, 1, 1) __launch_bounds__(kLWarps * 32, 1)
+__global__ void __cluster_dims__(kLCluster, 1, 1) __launch_bounds__(kLWarps * 32, kLCtasPerSm)
 unfold_long_f32_kernel(LongParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -195,7 +201,7 @@ unfold_long_f32_kernel(LongParams p)
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
     const int crank = (int)cluster_rank();
-    const int gw = crank * kLWarps + warp;                              // warp index within the station's team of 16
+    const int gw = crank * kLWarps + warp;                              // warp index within the station's team of 32
     const long cluster_id = blockIdx.x / kLCluster, n_clusters = gridDim.x / kLCluster;
     R *X = reinterpret_cast<R *>(smem + 8192 + 4096 + 128 + (size_t)warp * kXBytes);   // transpose plane / mirror rows
     R *Xpartner = reinterpret_cast<R *>(smem + 8192 + 4096 + 128 + (size_t)(warp ^ 1) * kXBytes);
@@ -441,7 +447,7 @@ static size_t long_stride(const PlanDev &p)
     const size_t C = (size_t)((p.k_hi >> 5) - (p.k_lo >> 5) + 1);
     return (kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | per-CTA peaks
 }
-size_t long_f32_scratch_bytes(const PlanDev &p) { return (148 / kLCluster) * long_stride(p); }
+size_t long_f32_scratch_bytes(const PlanDev &p) { return kLMaxClusters * long_stride(p); }
 
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                    void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
@@ -456,19 +462,30 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.C = (p.k_hi >> 5) - (p.k_lo >> 5) + 1;
     const size_t smem = 8192 + 4096 + 128 + (size_t)kLWarps * kXBytes;
-    const long grid = kLCluster * (n_units < 148 / kLCluster ? n_units : 148 / kLCluster);
     cudaError_t e;
-    if (efield) {
-        e = cudaFuncSetAttribute(unfold_long_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto launch = [&](auto kern) -> cudaError_t {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        unfold_long_f32_kernel<true><<<(unsigned)grid, kLWarps * 32, smem, s>>>(q);
-    } else {
-        e = cudaFuncSetAttribute(unfold_long_f32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        unfold_long_f32_kernel<false><<<(unsigned)grid, kLWarps * 32, smem, s>>>(q);
-    }
+        // persistent clusters: as many as can be co-resident (a cluster of 8 must fit one GPC), at most one per station
+        static int max_clusters = 0;                       // same for both instantiations to within rounding; cached
+        if (max_clusters == 0) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(kLCluster * kLMaxClusters); cfg.blockDim = dim3(kLWarps * 32); cfg.dynamicSmemBytes = smem;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = kLCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) { (void)cudaGetLastError(); n = kLMaxClusters; }
+            max_clusters = n < kLMaxClusters ? n : kLMaxClusters;
+            if (getenv("AERA_DEBUG")) fprintf(stderr, "[aera] long-trace kernel: %d co-resident clusters of %d CTAs (occupancy query %d)\n", max_clusters, kLCluster, n);
+        }
+        const long clusters = n_units < max_clusters ? n_units : max_clusters;
+        kern<<<(unsigned)(kLCluster * clusters), kLWarps * 32, smem, s>>>(q);
+        return cudaGetLastError();
+    };
+    e = efield ? launch(unfold_long_f32_kernel<true>) : launch(unfold_long_f32_kernel<false>);
     count_launches(1);
-    return cudaGetLastError();
+    return e;
 }
 
 } // namespace aera

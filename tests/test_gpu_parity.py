@@ -291,3 +291,29 @@ def test_full_size_config3(B, orc):
 
 def test_full_size_config4(B, orc):
     _full_size_case(B, orc, 4, 100, [0, 5000, 12399], n_canon=100)
+
+
+@pytest.mark.parametrize("cfg,n_events,n_st", [(1, 40, 124), (3, 30, 40), (4, 2, 124)])
+def test_repeated_runs_are_bit_identical(B, cfg, n_events, n_st):
+    """Race check by determinism (compute-sanitizer is not available on the GPU pool): the kernels have no
+    atomics on floating-point data, so repeated launches on the same input must agree bit for bit; a missing
+    barrier between the shared-memory / tensor-memory / L2-scratch phases would show up as a mismatch."""
+    wl = ai.WORKLOADS[cfg]
+    H = table_for(wl)
+    tr, dirs, _, _ = ai.make_batch(wl, range(min(n_events, 4)), n_stations=n_st)
+    reps = -(-n_events // tr.shape[0])
+    tr = np.concatenate([tr] * reps)[:n_events]; dirs = np.concatenate([dirs] * reps)[:n_events]
+    dt = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    try:
+        d_tr = torch.from_numpy(tr).cuda(); d_dirs = torch.from_numpy(dirs).cuda()
+        ref = None
+        for _ in range(6):
+            ef, amp, idx = B.aera_unfold_batch(pat, d_tr, d_dirs, wl.fs_hz)
+            torch.cuda.synchronize()
+            if ref is None:
+                ref = (ef.clone(), amp.clone(), idx.clone())
+            else:
+                assert torch.equal(ef, ref[0]) and torch.equal(amp, ref[1]) and torch.equal(idx, ref[2])
+    finally:
+        pat.free()
