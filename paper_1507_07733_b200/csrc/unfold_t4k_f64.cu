@@ -1,7 +1,7 @@
 // Team-per-station fused unfolding kernel for N = 4096 fp64 (BASELINE configs[3]).
 //
 // A "team" of 4 warps (128 threads x 32 complex doubles = 128 registers each) holds one station
-// entirely in registers; a CTA runs 3 teams (12 warps, one CTA per SM, persistent). Every long
+// entirely in registers; a CTA runs 2 teams (8 warps, one CTA per SM, persistent). Every long
 // transform is 4096 = 4 x 1024: a radix-4 step across the team plus one 1024-point FFT per warp
 // (32 x 32 in registers with one shared-memory transpose, fft32.cuh with plain double lanes).
 //
@@ -16,12 +16,16 @@
 //   a4 solve      : (E_theta, E_phi)[k] = Minv[event][k] (2V_0, 2V_1)[k] on the band rows, in registers;
 //                   Minv = (1/N) H^-1 (pattern.cu, once per event) is read through L1/L2 (64 KB per
 //                   event at configs[3], shared by the event's 40 stations).
-//   a5 inverse    : the band holds at most one bin per residue k mod 1024 (K <= 1024), so
-//                   z[4 m + s] = IFFT_1024 over k' of E[k(k')] W_4096^{-s k(k')}: warp s does sample
-//                   phase s, first theta then phi. E crosses the team once through shared memory.
+//   a5 inverse    : the mirror image of the forward path. Warp q inverse-transforms its OWN bins
+//                   Z[4 k' + q] (zero outside the band rows; E never leaves the registers / tensor memory),
+//                   multiplies u_q[m] by W_4096^{-m q}, the team exchanges, and the radix-4 step gives
+//                   z[m + 1024 s], s = 0..3, for this thread's 8 values of m: contiguous 8-byte stores.
+//                   theta first, then phi (E_phi waits in tensor memory).
 //   a6 outputs    : e_p[n] = Re z_p[n] from registers; |z_theta|^2 waits in this lane's tensor-memory
 //                   columns (tmem.cuh) for |z_phi|^2; running (max, lowest index) per lane, warp
 //                   shuffle argmax, then the 4 warps of the team combine through shared memory.
+//   twiddles      : the shared-memory pipe limits this kernel, so geometric twiddle sequences come from
+//                   two-term recurrences (reading R18) instead of table reads.
 //
 // HBM traffic per station: 64 KB read once, 64 KB + 12 B written once.
 // The in-band rows (bins k = 4 (lane + 32 row) + q) are template parameters: <4, 12> is configs[3]
@@ -35,7 +39,7 @@ namespace aera {
 namespace {
 
 using LD = LaneF64;
-constexpr int kTeams = 3;
+constexpr int kTeams = 2;                             // 8 warps x 250 registers: no spills; a third team (168 registers) was 2 % slower
 constexpr int kTeamThreads = 128;
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane
 constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B per team: exchange buffer / transpose planes / mirror rows
