@@ -317,3 +317,34 @@ def test_repeated_runs_are_bit_identical(B, cfg, n_events, n_st):
                 assert torch.equal(ef, ref[0]) and torch.equal(amp, ref[1]) and torch.equal(idx, ref[2])
     finally:
         pat.free()
+
+
+@pytest.mark.parametrize("cfg,n_st", [(3, 3), (4, 2)])
+def test_team_and_cluster_kernels_inplace_and_peaks_only(B, orc, cfg, n_st):
+    """The fp64 team kernel and the long-trace cluster kernel: E-field written over the input traces
+    (efield aliases traces), peaks only (efield NULL), and fewer stations than warps / teams / CTAs."""
+    wl = ai.WORKLOADS[cfg]
+    H = table_for(wl)
+    tr, dirs, _, _ = ai.make_batch(wl, [1], n_stations=n_st)
+    ref = oracle_batch(orc, wl, H, tr, dirs)
+    check(wl, run_gpu_batch(B, wl, H, tr, dirs, inplace=True), ref)
+    ef, amp, idx = run_gpu_batch(B, wl, H, tr, dirs, want_efield=False)
+    assert ef is None
+    check(wl, (None, amp, idx), ref)
+
+
+def test_scan_single_direction_and_station(B, orc):
+    wl = ai.WORKLOADS[2]
+    H = table_for(wl)
+    ev = ai.make_event(wl, 0)
+    for n_s, d_sel in ((1, [4242]), (2, [0, 7379]), (5, [17])):
+        tr = np.ascontiguousarray(ev.traces[:n_s]); dirs = ai.scan_directions()[d_sel]
+        pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+        try:
+            amp, idx = B.aera_scan_directions(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(dirs).cuda(), wl.fs_hz)
+            torch.cuda.synchronize()
+        finally:
+            pat.free()
+        oamp, oidx = orc.scan(wl.grid, H, wl.fs_hz, tr, dirs)
+        rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx)
+        assert rep.max_amp <= TOL["f32"]["amp"] and rep.idx_miss == 0, str(rep)
