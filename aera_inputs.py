@@ -174,8 +174,34 @@ class Event:
     pol_angle: np.ndarray  # [n_stations]
 
 
-def make_event(wl: Workload, event: int, n_stations: int | None = None) -> Event:
-    """Generate one event of workload `wl` (seed [7733, config, event])."""
+C_LIGHT_M_PER_S = 299792458.0
+
+
+def station_positions(n_stations: int = 124, spacing_m: float = 125.0, seed: int = 23) -> np.ndarray:
+    """[S][2] (x, y) in metres: a jittered square grid centred on the origin (stand-in for the AERA
+    layout of PAPER.md L23: 124 stations; the real positions are not available). With 125 m spacing the
+    array spans ~1.4 km, so at fs = 180 MHz a plane wave at 75 deg zenith spreads the arrival samples by
+    about +-400 around the trace centre."""
+    side = int(np.ceil(np.sqrt(n_stations)))
+    rng = np.random.default_rng([PATTERN_SEED, seed])
+    ij = np.stack(np.meshgrid(np.arange(side), np.arange(side), indexing="ij"), axis=-1).reshape(-1, 2)[:n_stations]
+    xy = (ij - (side - 1) / 2.0) * spacing_m + rng.uniform(-0.25, 0.25, size=(n_stations, 2)) * spacing_m
+    return np.ascontiguousarray(xy, dtype=np.float64)
+
+
+def plane_wave_arrival(wl: Workload, theta_deg: float, phi_deg: float, positions: np.ndarray) -> np.ndarray:
+    """Arrival sample of a plane wave coming FROM direction (theta, phi) at each station of a flat array:
+    n0_i = N/2 - fs (u x_i + v y_i) / c, (u, v) = sin(theta) (cos(phi), sin(phi)). Pure geometry of the inputs;
+    the method's own direction fit lives in the oracle and in the CUDA library."""
+    th, ph = np.deg2rad(theta_deg), np.deg2rad(phi_deg)
+    u, v = np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph)
+    return wl.n_samples / 2.0 - wl.fs_hz * (u * positions[:, 0] + v * positions[:, 1]) / C_LIGHT_M_PER_S
+
+
+def make_event(wl: Workload, event: int, n_stations: int | None = None, positions: np.ndarray | None = None) -> Event:
+    """Generate one event of workload `wl` (seed [7733, config, event]). With `positions` [S][2] the pulse
+    arrival samples follow a plane wave from the event direction (reconstruction-loop inputs) instead of
+    being drawn uniformly."""
     S = wl.n_stations if n_stations is None else n_stations
     N = wl.n_samples
     # config 2 is "one event drawn by the config-1 generator"
@@ -185,6 +211,8 @@ def make_event(wl: Workload, event: int, n_stations: int | None = None) -> Event
     phi = rng.uniform(0.0, 360.0)
     A = np.exp(rng.uniform(np.log(10.0), np.log(1000.0), size=S))
     n0 = rng.uniform(wl.arrival_lo, wl.arrival_hi, size=S)
+    if positions is not None:
+        n0 = plane_wave_arrival(wl, theta, phi, np.asarray(positions)[:S])
     psi = rng.uniform(0.0, 2 * np.pi, size=S)
     alpha = rng.uniform(0.0, 2 * np.pi, size=S)
 
