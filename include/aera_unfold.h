@@ -134,6 +134,38 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
                                    void *peak_amp, int32_t *peak_idx,
                                    void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/*
+ * Device-resident reconstruction loop (section 2, L29 and Fig. 1: "the maxima of the voltage
+ * traces are used as an initial guess on the signal timing and the direction is reconstructed from
+ * triangulation [...] the E-field trace at each station reconstructed [...] the maximum of the envelope
+ * [...] is used as updated timing information, and the process is iterated"; section 5, L83 names keeping
+ * the data on the GPU as the remedy for copy-dominated run time). Per event, all on the device:
+ *
+ *   n_i, w_i = lowest n maximising v0[n]^2 + v1[n]^2 and that maximum          (timing from the voltages)
+ *   for it = 0 .. n_iter-1:
+ *     (theta, phi) = weighted plane-wave fit of the arrival samples n_i on the flat array `positions`,
+ *                    c n_i / fs = c t0 - (u x_i + v y_i), (u, v) = sin(theta) (cos(phi), sin(phi)),
+ *                    weights w_i; theta = asin(min(1, |(u,v)|)), phi = atan2(v, u) in [0, 360) degrees;
+ *                    no positive weight or a degenerate array gives (0, 0)
+ *     unfold every station at (theta, phi) exactly as aera_unfold_batch does (peaks only, except that the
+ *     last iteration also writes the E-field traces when efield != NULL)
+ *     n_i = peak_idx_i, w_i = peak_amp_i^2
+ *
+ *   traces    [n_events][n_stations][2][n_samples] real (dtype)   device, 16-byte aligned
+ *   positions [n_stations][2] double, metres (x, y)                device
+ *   dirs_hist [n_iter][n_events][2] double, degrees                device, out
+ *   efield    as in aera_unfold_batch; may be NULL; may alias traces (written in the last iteration only)
+ *   amp_hist  [n_iter][n_events][n_stations] real (dtype), idx_hist the same shape int32     device, out
+ *   idx0 / w0 [n_events][n_stations] int32 / real (dtype): the voltage timing                 device, out
+ *   workspace as for aera_unfold_batch (AERA_OP_UNFOLD size for n_events)
+ * Asynchronous on the stream; errors as aera_unfold_batch, plus AERA_ERR_INVALID_ARG for n_iter < 1.
+ */
+aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                     int n_samples, double fs_hz, const void *traces, const double *positions,
+                                     int n_iter, double *dirs_hist, void *efield, void *amp_hist, int32_t *idx_hist,
+                                     int32_t *idx0, void *w0, void *workspace, size_t workspace_bytes,
+                                     void *cuda_stream);
+
 /* End-to-end convenience for HOST buffers (the paper's situation: traces live on
  * the host and are copied for every transform).  Same arguments as aera_unfold_batch but every
  * data pointer is a HOST pointer (page-locked memory gives full PCIe speed; pageable works).

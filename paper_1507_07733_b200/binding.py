@@ -20,7 +20,7 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
           4: "AERA_ERR_WORKSPACE", 5: "AERA_ERR_ALLOC", 6: "AERA_ERR_CUDA", 7: "AERA_ERR_BAND"}
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
-           "aera_scan_directions", "aera_unfold_batch_host", "aera_set_kernel_variant", "aera_launch_count",
+           "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read")
 
 
@@ -67,6 +67,9 @@ def _load():
     lib.aera_scan_directions.restype = C.c_int
     lib.aera_unfold_batch_host.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp]
     lib.aera_unfold_batch_host.restype = C.c_int
+    lib.aera_reconstruct_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, C.c_int, dp, vp, vp, vp, vp, vp,
+                                           vp, C.c_size_t, vp]
+    lib.aera_reconstruct_batch.restype = C.c_int
     lib.aera_set_kernel_variant.argtypes = [C.c_int]
     lib.aera_set_kernel_variant.restype = C.c_int
     lib.aera_launch_count.restype = C.c_ulonglong
@@ -143,7 +146,7 @@ def aera_set_kernel_variant(variant: int) -> int:
     return int(_lib.aera_set_kernel_variant(int(variant)))
 
 
-KERNEL_IDS = {"repack": 0, "minv": 1, "unfold": 2, "scan_fwd": 3, "scan_inv": 4}
+KERNEL_IDS = {"repack": 0, "minv": 1, "unfold": 2, "scan_fwd": 3, "scan_inv": 4, "timing": 5, "planefit": 6}
 
 
 def aera_profile_enable(on: bool) -> int:
@@ -234,6 +237,30 @@ def aera_scan_directions(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, f
     _check(_lib.aera_scan_directions(p.handle, dt, S, N, fs_hz, _ptr(traces), D, _ptr(dirs), _ptr(peak_amp), _ptr(peak_idx),
                                      _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
     return peak_amp, peak_idx
+
+
+def aera_reconstruct_batch(p: Pattern, traces: torch.Tensor, positions: torch.Tensor, fs_hz: float, n_iter: int,
+                           efield=None, want_efield=True, workspace=None, stream=None):
+    """traces [E][S][2][N] CUDA, positions [S][2] CUDA float64 (metres). Returns a dict with dirs_hist
+    [n_iter][E][2], efield (or None), amp_hist / idx_hist [n_iter][E][S], idx0 / w0 [E][S]."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    assert positions.is_cuda and positions.dtype == torch.float64 and tuple(positions.shape) == (S, 2) and positions.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    dev = traces.device
+    if efield is None and want_efield:
+        efield = torch.empty_like(traces)
+    dirs_hist = torch.empty((n_iter, E, 2), dtype=torch.float64, device=dev)
+    amp_hist = torch.empty((n_iter, E, S), dtype=traces.dtype, device=dev)
+    idx_hist = torch.empty((n_iter, E, S), dtype=torch.int32, device=dev)
+    idx0 = torch.empty((E, S), dtype=torch.int32, device=dev)
+    w0 = torch.empty((E, S), dtype=traces.dtype, device=dev)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, dev)
+    _check(_lib.aera_reconstruct_batch(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(positions), n_iter, _ptr(dirs_hist),
+                                       _ptr(efield) if efield is not None else None, _ptr(amp_hist), _ptr(idx_hist), _ptr(idx0), _ptr(w0),
+                                       _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return dict(dirs_hist=dirs_hist, efield=efield, amp_hist=amp_hist, idx_hist=idx_hist, idx0=idx0, w0=w0)
 
 
 def aera_unfold_batch_host(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, efield=None, peak_amp=None,

@@ -33,7 +33,7 @@ void count_launches(unsigned n);
 int kernel_variant();
 
 // Optional per-kernel CUDA-event timing (aera_profile_enable / aera_profile_read in the C ABI).
-enum KernelId { KID_REPACK = 0, KID_MINV = 1, KID_UNFOLD = 2, KID_SCAN_FWD = 3, KID_SCAN_INV = 4, KID_COUNT = 5 };
+enum KernelId { KID_REPACK = 0, KID_MINV = 1, KID_UNFOLD = 2, KID_SCAN_FWD = 3, KID_SCAN_INV = 4, KID_TIMING = 5, KID_PLANEFIT = 6, KID_COUNT = 7 };
 void prof_begin(int kid, cudaStream_t s); // no-ops unless profiling is enabled
 void prof_end(int kid, cudaStream_t s);
 struct ProfScope {
@@ -85,6 +85,11 @@ bool long_f32_supported(int dtype, const PlanDev &p);
 size_t long_f32_scratch_bytes(const PlanDev &p);
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                    void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s);
+
+// ---- loop.cu: the two small steps that close the reconstruction loop on the device
+cudaError_t launch_timing(int dtype, const void *traces, long n_units, int N, int32_t *idx0, void *w0, cudaStream_t s);
+cudaError_t launch_planefit(int dtype, const double *pos, const int32_t *idx, const void *w, int square_w, long n_events,
+                            int n_stations, double fs, double *dirs, cudaStream_t s);
 
 // ---- scan_w32.cu: direction scan for N = 2048 fp32, band rows 10..28 (configs[2])
 bool scan_w32_supported(int dtype, const PlanDev &p);

@@ -463,6 +463,43 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
     return AERA_OK;
 }
 
+aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                     int n_samples, double fs_hz, const void *traces, const double *positions,
+                                     int n_iter, double *dirs_hist, void *efield, void *amp_hist, int32_t *idx_hist,
+                                     int32_t *idx0, void *w0, void *workspace, size_t workspace_bytes,
+                                     void *cuda_stream)
+{
+    aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
+    if (st != AERA_OK) return st;
+    if (n_events < 0) return fail(AERA_ERR_INVALID_ARG, "n_events=%d is negative", n_events);
+    if (n_iter < 1) return fail(AERA_ERR_INVALID_ARG, "n_iter=%d must be at least 1", n_iter);
+    if (n_events == 0) return AERA_OK;
+    if (!traces || !positions || !dirs_hist || !amp_hist || !idx_hist || !idx0 || !w0)
+        return fail(AERA_ERR_INVALID_ARG, "traces, positions, dirs_hist, amp_hist, idx_hist, idx0 and w0 must be non-NULL");
+    if (misaligned(traces, 16) || misaligned(positions, 8) || misaligned(dirs_hist, 8))
+        return fail(AERA_ERR_INVALID_ARG, "traces must be 16-byte aligned, positions and dirs_hist 8-byte aligned");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t rb = real_bytes(dtype);
+    const size_t units = (size_t)n_events * n_stations;
+    cudaError_t e = launch_timing(dtype, traces, (long)units, n_samples, idx0, w0, s);
+    if (e != cudaSuccess) return cuda_fail(e, "timing kernel launch");
+    const int32_t *t_idx = idx0;
+    const void *t_w = w0;
+    int square = 0;
+    for (int it = 0; it < n_iter; ++it) {
+        double *dirs = dirs_hist + (size_t)it * n_events * 2;
+        e = launch_planefit(dtype, positions, t_idx, t_w, square, n_events, n_stations, fs_hz, dirs, s);
+        if (e != cudaSuccess) return cuda_fail(e, "plane-wave fit kernel launch");
+        void *amp = static_cast<unsigned char *>(amp_hist) + (size_t)it * units * rb;
+        int32_t *idx = idx_hist + (size_t)it * units;
+        st = aera_unfold_batch(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs,
+                               it == n_iter - 1 ? efield : nullptr, amp, idx, workspace, workspace_bytes, cuda_stream);
+        if (st != AERA_OK) return st;
+        t_idx = idx; t_w = amp; square = 1;
+    }
+    return AERA_OK;
+}
+
 aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
                                      int n_samples, double fs_hz, const void *traces_host,
                                      const double *dirs_host, void *efield_host, void *peak_amp_host,

@@ -1,0 +1,89 @@
+"""GPU parity of the device-resident reconstruction loop (aera_reconstruct_batch) against the loop oracle
+(oracle/aera_loop.py). Every step is checked on the GPU's own inputs of that step, so one admissible
+near-tie (a peak index off by one) cannot cascade into the later comparisons: where floating point decides
+an integer both sides must agree or be a near-tie; given the same integers and weights, the double-precision
+fit must agree to rounding."""
+import numpy as np
+import pytest
+import torch
+
+import aera_inputs as ai
+from parity import TOL, compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import paper_1507_07733_b200.binding as b
+    assert torch.cuda.is_available()
+    return b
+
+
+def _ang(a, b):
+    return abs((a - b + 180.0) % 360.0 - 180.0)
+
+
+@pytest.mark.parametrize("cfg,n_events,n_st,n_iter", [(1, 5, 124, 3), (0, 2, 7, 2), (3, 3, 40, 2)])
+def test_reconstruct_batch_step_by_step(B, cfg, n_events, n_st, n_iter):
+    import oracle
+    from oracle import aera_loop as ol
+    wl = ai.WORKLOADS[cfg]
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    spacing = 125.0 if cfg != 0 else 40.0          # configs[0]: 256 samples at 200 MHz only span ~190 m
+    pos = ai.station_positions(n_st, spacing_m=spacing if cfg != 3 else 100.0)
+    evs = [ai.make_event(wl, e, n_stations=n_st, positions=pos) for e in range(n_events)]
+    tr = np.stack([e.traces for e in evs])
+    dt = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    try:
+        g = B.aera_reconstruct_batch(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(pos).cuda(), wl.fs_hz, n_iter)
+        torch.cuda.synchronize()
+        g = {k: (v.cpu().numpy() if v is not None else None) for k, v in g.items()}
+    finally:
+        pat.free()
+    tie = TOL[wl.dtype]["tie"]
+    for e in range(n_events):
+        # timing from the voltages: exact unless the two maxima are a near-tie
+        o_idx0, o_w0 = ol.timing_from_voltages(tr[e])
+        p = tr[e, :, 0, :].astype(np.float64) ** 2 + tr[e, :, 1, :].astype(np.float64) ** 2
+        for s in range(n_st):
+            if g["idx0"][e, s] != o_idx0[s]:
+                assert 1.0 - p[s, g["idx0"][e, s]] / p[s, o_idx0[s]] < tie, (e, s)
+        assert np.allclose(g["w0"][e], o_w0, rtol=10 * TOL[wl.dtype]["amp"])
+        t, w = g["idx0"][e].astype(np.float64), g["w0"][e].astype(np.float64)
+        for it in range(n_iter):
+            th_o, ph_o = ol.planewave_fit(pos, t, w, wl.fs_hz)      # the oracle's fit on the GPU's integers / weights
+            th_g, ph_g = g["dirs_hist"][it, e]
+            assert abs(th_g - th_o) < 1e-8 and _ang(ph_g, ph_o) < 1e-8 / max(np.sin(np.deg2rad(th_o)), 1e-3), (e, it, th_g, th_o, ph_g, ph_o)
+            ref = oracle.unfold_batch(wl.grid, H, wl.fs_hz, tr[e], np.tile([th_g, ph_g], (n_st, 1)), want_env2=True)
+            last = it == n_iter - 1
+            rep = compare(wl.dtype, g["efield"][e] if last else None, g["amp_hist"][it, e], g["idx_hist"][it, e], ref)
+            assert rep.ok(TOL[wl.dtype]), f"event {e} iteration {it}: {rep}"
+            t, w = g["idx_hist"][it, e].astype(np.float64), g["amp_hist"][it, e].astype(np.float64) ** 2
+        # plausibility: the loop ends near the injected direction
+        th0, ph0 = evs[e].direction_deg
+        # (in sin(theta): at large zenith angles a small error of the fitted (u, v) is a large one in theta)
+        assert abs(np.sin(np.deg2rad(g["dirs_hist"][-1, e, 0])) - np.sin(np.deg2rad(th0))) < 0.06, (e, g["dirs_hist"][:, e], th0, ph0)
+
+
+def test_reconstruct_batch_errors_and_inplace(B):
+    wl = ai.WORKLOADS[1]
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    pos = ai.station_positions(12)
+    ev = ai.make_event(wl, 0, n_stations=12, positions=pos)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        tr = torch.from_numpy(ev.traces[None]).cuda()
+        with pytest.raises(B.AeraError) as e:
+            B.aera_reconstruct_batch(pat, tr, torch.from_numpy(pos).cuda(), wl.fs_hz, 0)
+        assert e.value.status == 1
+        a = B.aera_reconstruct_batch(pat, tr, torch.from_numpy(pos).cuda(), wl.fs_hz, 2)
+        b = B.aera_reconstruct_batch(pat, tr.clone(), torch.from_numpy(pos).cuda(), wl.fs_hz, 2, want_efield=False)
+        tr2 = tr.clone()
+        c = B.aera_reconstruct_batch(pat, tr2, torch.from_numpy(pos).cuda(), wl.fs_hz, 2, efield=tr2)   # in place
+        torch.cuda.synchronize()
+        assert b["efield"] is None and torch.equal(a["idx_hist"], b["idx_hist"]) and torch.equal(a["dirs_hist"], b["dirs_hist"])
+        assert torch.equal(c["efield"], a["efield"]) and torch.equal(c["amp_hist"], a["amp_hist"])
+    finally:
+        pat.free()
