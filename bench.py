@@ -302,6 +302,66 @@ def run_loop(args, wl):
     pat.free()
 
 
+
+def run_fold(args, wl):
+    """--fold: aera_fold_batch on the config's shapes: seeded white E-field traces in, voltage
+    traces out; same fused kernels as the unfold with (1/N) H as the matrix, so the same algorithmic bytes."""
+    import torch
+    import paper_1507_07733_b200.binding as B
+    torch.cuda.set_device(0)
+    n_events = args.events or (wl.n_events if wl.config != 3 else 2000)
+    dt_code = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt_code), H)
+    g = torch.Generator(device="cuda"); g.manual_seed(7733)
+    d_ef = torch.randn((n_events, wl.n_stations, 2, wl.n_samples), generator=g, device="cuda", dtype=torch.float32 if wl.dtype == "f32" else torch.float64)
+    rng = np.random.default_rng(7733)
+    d_dirs = torch.from_numpy(np.stack([rng.uniform(0, wl.zenith_max_deg, n_events), rng.uniform(0, 360, n_events)], axis=1)).cuda()
+    d_tr = torch.empty_like(d_ef)
+    ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_FOLD, pat, dt_code, n_events, wl.n_stations, wl.n_samples, wl.fs_hz))
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.aera_fold_batch(pat, d_ef, d_dirs, wl.fs_hz, traces=d_tr, workspace=ws, stream=stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0); sampler.start()
+    B.aera_profile_enable(True)
+    l0 = B.aera_launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / args.steps
+    launches = B.aera_launch_count() - l0
+    B.aera_profile_enable(False)
+    k_ms, k_n = B.aera_profile_read(B.KERNEL_IDS["unfold"])
+    clocks = sampler.stop()
+    n_units = n_events * wl.n_stations
+    peak, peak_src = load_peaks()
+    b_unit = algorithmic_bytes_per_unit(wl)
+    k_avg = k_ms / max(k_n, 1)
+    achieved = n_units * b_unit / (k_avg * 1e-3) / 1e9
+    line = {
+        "metric": "station-traces folded/sec (forward model V = H E on the device)", "value": n_units / (ms_step * 1e-3), "unit": UNIT, "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": wl.dtype, "data": "synthetic (seeded white E-field traces generated on the device)",
+        "config": {"workload": f"BASELINE configs[{wl.config}] shapes, forward model: {n_events} events x {wl.n_stations} stations x 2 x {wl.n_samples} {wl.dtype}",
+                   "n_events": n_events, "l2_policy": f"inputs+outputs {2 * d_ef.numel() * d_ef.element_size() / 1e9:.1f} GB >> 126 MB L2"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "kernel": "unfold kernels with the forward matrix", "kernel_ms": k_avg, "kernel_share_of_step": k_avg / ms_step,
+                     "algorithmic_bytes_per_unit": b_unit, "peak_source": peak_src},
+        "cpu_baseline": None, "e2e": None, "gpu_launches": int(launches), "clocks": clocks,
+        "outputs_sane": bool(torch.isfinite(d_tr).all().item()), "library": B.aera_version(),
+    }
+    print(json.dumps(line), flush=True)
+    pat.free()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -312,6 +372,7 @@ def main():
     ap.add_argument("--events", type=int, default=0, help="override the number of events (0 = the config's)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 auto, 1 generic)")
     ap.add_argument("--loop", type=int, default=0, help="config 1 only: time the device-resident reconstruction loop with this many iterations")
+    ap.add_argument("--fold", action="store_true", help="time the on-device forward model (aera_fold_batch) on the config's shapes")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -325,6 +386,10 @@ def main():
     if args.config == 2:
         if int(os.environ.get("RANK", "0")) == 0:
             run_scan(args, wl)
+        return
+    if args.fold:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_fold(args, wl)
         return
     if args.loop > 0:
         if args.config != 1:

@@ -92,7 +92,7 @@ aera_status_t aera_pattern_free(aera_pattern_t *pattern);
 aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_hz,
                         int *k_lo, int *k_hi);
 
-typedef enum { AERA_OP_UNFOLD = 0, AERA_OP_SCAN = 1 } aera_op_t;
+typedef enum { AERA_OP_UNFOLD = 0, AERA_OP_SCAN = 1, AERA_OP_FOLD = 2 } aera_op_t;
 
 /* Scratch bytes needed by aera_unfold_batch (n_events_or_dirs = n_events) or
  * aera_scan_directions (n_events_or_dirs = n_dirs) for these sizes; 0 on invalid arguments
@@ -133,6 +133,24 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
                                    long n_dirs, const double *dirs,
                                    void *peak_amp, int32_t *peak_idx,
                                    void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * Forward model on the device (the inverse of the solve of aera_unfold_batch; section 3: the
+ * voltage of each channel is the vector effective length applied to the electric field vector): for every
+ * station, with the event's direction,
+ *     E_p[k]  = sum_n e_p[n] exp(-2 pi i n k / N),  p = theta, phi
+ *     V_c[k]  = H_c,theta[k] E_theta[k] + H_c,phi[k] E_phi[k]   on the table band, 0 elsewhere (and at DC, Nyquist)
+ *     v_c[n]  = (2/N) Re sum_{k in band} V_c[k] exp(+2 pi i n k / N)
+ * i.e. the band-limited E-field folded with the interpolated antenna response. It runs the same fused
+ * kernels as aera_unfold_batch with the matrix (1/N) H in place of (1/N) H^-1.
+ *   efield [n_events][n_stations][2 (theta, phi)][n_samples] real, device, in
+ *   dirs   [n_events][2] double degrees, device
+ *   traces [n_events][n_stations][2 (channels)][n_samples] real, device, out; may alias efield
+ *   workspace >= aera_workspace_bytes(AERA_OP_FOLD, ...)
+ */
+aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                              int n_samples, double fs_hz, const void *efield, const double *dirs,
+                              void *traces, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
  * Device-resident reconstruction loop (section 2, L29 and Fig. 1: "the maxima of the voltage

@@ -15,12 +15,12 @@ import torch
 from . import build as _build
 
 AERA_F32, AERA_F64 = 0, 1
-AERA_OP_UNFOLD, AERA_OP_SCAN = 0, 1
+AERA_OP_UNFOLD, AERA_OP_SCAN, AERA_OP_FOLD = 0, 1, 2
 STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 3: "AERA_ERR_DTYPE_MISMATCH",
           4: "AERA_ERR_WORKSPACE", 5: "AERA_ERR_ALLOC", 6: "AERA_ERR_CUDA", 7: "AERA_ERR_BAND"}
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
-           "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_set_kernel_variant", "aera_launch_count",
+           "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read")
 
 
@@ -70,6 +70,8 @@ def _load():
     lib.aera_reconstruct_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, C.c_int, dp, vp, vp, vp, vp, vp,
                                            vp, C.c_size_t, vp]
     lib.aera_reconstruct_batch.restype = C.c_int
+    lib.aera_fold_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, C.c_size_t, vp]
+    lib.aera_fold_batch.restype = C.c_int
     lib.aera_set_kernel_variant.argtypes = [C.c_int]
     lib.aera_set_kernel_variant.restype = C.c_int
     lib.aera_launch_count.restype = C.c_ulonglong
@@ -237,6 +239,21 @@ def aera_scan_directions(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, f
     _check(_lib.aera_scan_directions(p.handle, dt, S, N, fs_hz, _ptr(traces), D, _ptr(dirs), _ptr(peak_amp), _ptr(peak_idx),
                                      _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
     return peak_amp, peak_idx
+
+
+def aera_fold_batch(p: Pattern, efield: torch.Tensor, dirs: torch.Tensor, fs_hz: float, traces=None, workspace=None, stream=None):
+    """efield [E][S][2 (theta, phi)][N] CUDA, dirs [E][2] CUDA float64 -> voltage traces [E][S][2][N] (forward model)."""
+    E, S, two, N = efield.shape
+    assert two == 2 and efield.is_cuda and efield.is_contiguous()
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    dt = _dtype_code(efield.dtype)
+    if traces is None:
+        traces = torch.empty_like(efield)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_FOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, efield.device)
+    _check(_lib.aera_fold_batch(p.handle, dt, E, S, N, fs_hz, _ptr(efield), _ptr(dirs), _ptr(traces), _ptr(workspace),
+                                workspace.numel(), _stream_ptr(stream)))
+    return traces
 
 
 def aera_reconstruct_batch(p: Pattern, traces: torch.Tensor, positions: torch.Tensor, fs_hz: float, n_iter: int,

@@ -57,7 +57,8 @@ enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3 };
 // complex elements per direction in the MINV_Q4 layout (<= 4 K + 32)
 __host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
-                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s);
+                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s,
+                        int forward = 0 /* 1: scale * H (forward model) instead of scale * H^-1 */);
 size_t minv_smem_bytes(int dtype, int n_f);
 
 // ---- unfold_generic.cu

@@ -230,7 +230,7 @@ TableGeom geom_of(const aera_pattern_desc_t &d)
 }
 
 struct WsLayout {
-    size_t off_minv, off_scratch, off_spectra, total;
+    size_t off_minv, off_scratch, off_spectra, off_peaks, total;
 };
 
 // Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
@@ -246,7 +246,7 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
     if (q32 > per_dir) per_dir = q32;
     w.off_minv = o; o = align_up(o + (size_t)n_dirs * per_dir * cb);
     size_t scratch = generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations);
-    if (op == AERA_OP_UNFOLD && long_f32_supported(dtype, band) && long_f32_scratch_bytes(band) > scratch)
+    if (op != AERA_OP_SCAN && long_f32_supported(dtype, band) && long_f32_scratch_bytes(band) > scratch)
         scratch = long_f32_scratch_bytes(band);
     w.off_scratch = o; o = align_up(o + scratch);
     w.off_spectra = o;
@@ -254,6 +254,8 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
         size_t a = generic_scan_spectra_bytes(dtype, K, n_stations), b = scan_w32_spectra_bytes(n_stations);
         o = align_up(o + (a > b ? a : b));
     }
+    w.off_peaks = o;                                                      // fold: the by-product peaks of the shared kernels
+    if (op == AERA_OP_FOLD) o = align_up(o + (size_t)n_dirs * n_stations * 12);
     w.total = o > 0 ? o : kAlign;
     return w;
 }
@@ -375,7 +377,7 @@ aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_
 size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,
                             int n_stations, int n_samples, double fs_hz)
 {
-    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
+    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN && op != AERA_OP_FOLD) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
     if (check_common(pattern, dtype, n_stations, n_samples, fs_hz) != AERA_OK) return 0;
     if (n_events_or_dirs < 0) { fail(AERA_ERR_INVALID_ARG, "negative count"); return 0; }
     int k_lo, k_hi;
@@ -383,27 +385,34 @@ size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dty
     return ws_layout(op, dtype, n_samples, k_lo, k_hi - k_lo + 1, n_events_or_dirs, n_stations).total;
 }
 
-aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
-                                int n_samples, double fs_hz, const void *traces, const double *dirs,
-                                void *efield, void *peak_amp, int32_t *peak_idx,
-                                void *workspace, size_t workspace_bytes, void *cuda_stream)
+// aera_unfold_batch (forward = 0) and aera_fold_batch (forward = 1: the same kernels with (1/N) H in place of
+// (1/N) H^-1, peaks into the workspace)
+static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                 int n_samples, double fs_hz, const void *traces, const double *dirs,
+                                 void *efield, void *peak_amp, int32_t *peak_idx,
+                                 void *workspace, size_t workspace_bytes, void *cuda_stream, int forward)
 {
     aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
     if (st != AERA_OK) return st;
     if (n_events < 0) return fail(AERA_ERR_INVALID_ARG, "n_events=%d is negative", n_events);
     if (n_events == 0) return AERA_OK;
-    if (!traces || !dirs || !peak_amp || !peak_idx) return fail(AERA_ERR_INVALID_ARG, "traces, dirs, peak_amp and peak_idx must be non-NULL");
+    if (!traces || !dirs || (!forward && (!peak_amp || !peak_idx)) || (forward && !efield))
+        return fail(AERA_ERR_INVALID_ARG, forward ? "efield, dirs and traces must be non-NULL" : "traces, dirs, peak_amp and peak_idx must be non-NULL");
     if (misaligned(traces, 16) || (efield && misaligned(efield, 16))) return fail(AERA_ERR_INVALID_ARG, "traces and efield must be 16-byte aligned");
-    if (misaligned(dirs, 8) || misaligned(peak_amp, real_bytes(dtype)) || misaligned(peak_idx, 4))
+    if (misaligned(dirs, 8) || (!forward && (misaligned(peak_amp, real_bytes(dtype)) || misaligned(peak_idx, 4))))
         return fail(AERA_ERR_INVALID_ARG, "dirs / peak_amp / peak_idx are not aligned to their element size");
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     Plan *pl = nullptr;
     st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
     if (st != AERA_OK) return st;
-    const WsLayout w = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, n_events, n_stations);
+    const WsLayout w = ws_layout(forward ? AERA_OP_FOLD : AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, n_events, n_stations);
     if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
+    if (forward) { // the kernels' envelope peaks are a by-product here: they go to the workspace
+        peak_amp = ws + w.off_peaks;
+        peak_idx = reinterpret_cast<int32_t *>(ws + w.off_peaks + (size_t)n_events * n_stations * 8);
+    }
 
     const bool warp_path = kernel_variant() == 0 && w32_supported(dtype, pl->dev);
     const bool team_path = kernel_variant() == 0 && t4k_f64_supported(dtype, pl->dev);
@@ -411,7 +420,7 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
     // the warp and team kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
                                 warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS)),
-                                ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s);
+                                ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s, forward);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
@@ -425,6 +434,24 @@ aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_
                                   ws + w.off_minv, ws + w.off_scratch, s);
     if (e != cudaSuccess) return cuda_fail(e, "unfold kernel launch");
     return AERA_OK;
+}
+
+aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                int n_samples, double fs_hz, const void *traces, const double *dirs,
+                                void *efield, void *peak_amp, int32_t *peak_idx,
+                                void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    return unfold_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs, efield, peak_amp, peak_idx,
+                       workspace, workspace_bytes, cuda_stream, 0);
+}
+
+aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                              int n_samples, double fs_hz, const void *efield, const double *dirs,
+                              void *traces, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    // the kernels read their "traces" argument and write their "efield" argument: swapped roles here
+    return unfold_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, efield, dirs, traces, nullptr, nullptr,
+                       workspace, workspace_bytes, cuda_stream, 1);
 }
 
 aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int n_stations, int n_samples,

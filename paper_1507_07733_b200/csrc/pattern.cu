@@ -92,7 +92,7 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restrict__ dirs,
             const int *__restrict__ bin_if, const double *__restrict__ bin_tf, int K, double scale,
-            int layout, int k_lo, cx<T> *__restrict__ minv)
+            int layout, int k_lo, int forward, cx<T> *__restrict__ minv)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
@@ -150,6 +150,10 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         mt1.re = (T)(-(hr[1] * ir - hi[1] * ii)); mt1.im = (T)(-(hr[1] * ii + hi[1] * ir));
         mp0.re = (T)(-(hr[2] * ir - hi[2] * ii)); mp0.im = (T)(-(hr[2] * ii + hi[2] * ir));
         mp1.re = (T)(hr[0] * ir - hi[0] * ii);    mp1.im = (T)(hr[0] * ii + hi[0] * ir);
+        if (forward) { // the forward model (aera_fold_batch): scale * H itself, rows (V0 <- E_theta, V0 <- E_phi, V1 <- E_theta, V1 <- E_phi)
+            mt0.re = (T)(scale * hr[0]); mt0.im = (T)(scale * hi[0]); mt1.re = (T)(scale * hr[1]); mt1.im = (T)(scale * hi[1]);
+            mp0.re = (T)(scale * hr[2]); mp0.im = (T)(scale * hi[2]); mp1.re = (T)(scale * hr[3]); mp1.im = (T)(scale * hi[3]);
+        }
         if (layout == MINV_ROWS) {
             o[0] = mt0; o[1] = mt1; o[2] = mp0; o[3] = mp1;
         } else if (layout == MINV_Q4) {
@@ -178,7 +182,7 @@ size_t minv_smem_bytes(int dtype, int n_f)
 }
 
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
-                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s)
+                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s, int forward)
 {
     if (n_dirs <= 0) return cudaSuccess;
     ProfScope prof(KID_MINV, s);
@@ -188,12 +192,12 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
         e = cudaFuncSetAttribute(minv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                             p.K, scale, layout, p.k_lo, (cx<float> *)minv);
+                                                             p.K, scale, layout, p.k_lo, forward, (cx<float> *)minv);
     } else {
         e = cudaFuncSetAttribute(minv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf,
-                                                              p.K, scale, layout, p.k_lo, (cx<double> *)minv);
+                                                              p.K, scale, layout, p.k_lo, forward, (cx<double> *)minv);
     }
     count_launches(1);
     return cudaGetLastError();
