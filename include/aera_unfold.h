@@ -135,6 +135,19 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
                                    void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * Optional pre-filter fused into the unfolding (section 2: "noise filtering and signal
+ * enhancing" precedes the loop; the paper does not specify the filter). One real weight per in-band DFT
+ * bin k_lo .. k_hi of a given (n_samples, fs_hz) (aera_band gives the range; n_weights must equal
+ * k_hi - k_lo + 1): E[k] = weights[k - k_lo] * H[k]^-1 V[k], e.g. a band-pass taper or notches at narrow-band
+ * transmitters. The weights are folded into the per-direction matrices, so the filter costs nothing per
+ * station. It applies to aera_unfold_batch, aera_scan_directions and aera_reconstruct_batch of this pattern
+ * for that (n_samples, fs_hz) until replaced; weights == NULL removes it. aera_fold_batch ignores it.
+ * weights is a HOST pointer; the call synchronises the stream (it is a configuration call, not a hot one).
+ */
+aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_samples, double fs_hz, const double *weights,
+                                           int n_weights, void *cuda_stream);
+
+/*
  * Forward model on the device (the inverse of the solve of aera_unfold_batch; section 3: the
  * voltage of each channel is the vector effective length applied to the electric field vector): for every
  * station, with the event's direction,

@@ -20,7 +20,7 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
           4: "AERA_ERR_WORKSPACE", 5: "AERA_ERR_ALLOC", 6: "AERA_ERR_CUDA", 7: "AERA_ERR_BAND"}
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
-           "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_set_kernel_variant", "aera_launch_count",
+           "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read")
 
 
@@ -72,6 +72,8 @@ def _load():
     lib.aera_reconstruct_batch.restype = C.c_int
     lib.aera_fold_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, C.c_size_t, vp]
     lib.aera_fold_batch.restype = C.c_int
+    lib.aera_pattern_set_band_filter.argtypes = [vp, C.c_int, C.c_double, dp, C.c_int, vp]
+    lib.aera_pattern_set_band_filter.restype = C.c_int
     lib.aera_set_kernel_variant.argtypes = [C.c_int]
     lib.aera_set_kernel_variant.restype = C.c_int
     lib.aera_launch_count.restype = C.c_ulonglong
@@ -239,6 +241,15 @@ def aera_scan_directions(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, f
     _check(_lib.aera_scan_directions(p.handle, dt, S, N, fs_hz, _ptr(traces), D, _ptr(dirs), _ptr(peak_amp), _ptr(peak_idx),
                                      _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
     return peak_amp, peak_idx
+
+
+def aera_pattern_set_band_filter(p: Pattern, n_samples: int, fs_hz: float, weights, stream=None):
+    """weights: 1-D array-like of length K (host) or None to remove the filter."""
+    if weights is None:
+        _check(_lib.aera_pattern_set_band_filter(p.handle, n_samples, fs_hz, None, 0, _stream_ptr(stream)))
+        return
+    w = np.ascontiguousarray(weights, dtype=np.float64)
+    _check(_lib.aera_pattern_set_band_filter(p.handle, n_samples, fs_hz, w.ctypes.data_as(C.c_void_p), int(w.size), _stream_ptr(stream)))
 
 
 def aera_fold_batch(p: Pattern, efield: torch.Tensor, dirs: torch.Tensor, fs_hz: float, traces=None, workspace=None, stream=None):

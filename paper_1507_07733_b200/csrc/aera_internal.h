@@ -24,6 +24,7 @@ struct PlanDev {
     int k_lo, k_hi, K;
     const int *bin_if;      // [K] lower frequency node of bin k_lo+j
     const double *bin_tf;   // [K] weight of the upper node
+    const double *bin_w;    // [K] optional pre-filter weight per in-band bin (NULL = none), folded into Minv
     const void *tw;         // [N/2] cx<T>: W_N^m = exp(-2 pi i m / N), m < N/2 (generic kernel)
     const void *tw1024;     // [1024] cx<T>: W_1024^m (warp kernels: 32x32 inter-pass twiddles)
     const void *twN;        // [N] cx<T>: W_N^m, m < N (real-FFT split / polyphase twiddles)

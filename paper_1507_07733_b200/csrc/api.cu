@@ -71,6 +71,7 @@ struct Plan {
     PlanDev dev{};
     double fs = 0;
     void *blob = nullptr; // one device allocation holding every table of the plan
+    double *d_filter = nullptr; // optional per-bin pre-filter weights (aera_pattern_set_band_filter)
 };
 
 struct HostPipe { // staging for aera_unfold_batch_host
@@ -351,7 +352,7 @@ aera_status_t aera_pattern_upload(const aera_pattern_desc_t *desc, const void *H
 aera_status_t aera_pattern_free(aera_pattern_t *p)
 {
     if (!p) return AERA_OK;
-    for (auto &kv : p->plans) { cudaFree(kv.second->blob); delete kv.second; }
+    for (auto &kv : p->plans) { cudaFree(kv.second->blob); cudaFree(kv.second->d_filter); delete kv.second; }
     HostPipe &hp = p->pipe;
     for (int i = 0; i < 2; ++i) {
         cudaFree(hp.d_in[i]); cudaFree(hp.d_out[i]); cudaFree(hp.d_amp[i]); cudaFree(hp.d_idx[i]);
@@ -372,6 +373,34 @@ aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_
     aera_status_t st = check_n(n_samples);
     if (st != AERA_OK) return st;
     return compute_band(pattern->desc, n_samples, fs_hz, k_lo, k_hi);
+}
+
+aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_samples, double fs_hz, const double *weights,
+                                           int n_weights, void *cuda_stream)
+{
+    if (!pattern) return fail(AERA_ERR_INVALID_ARG, "pattern is NULL");
+    aera_status_t st = check_n(n_samples);
+    if (st != AERA_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Plan *pl = nullptr;
+    st = get_plan(pattern, n_samples, fs_hz, s, &pl);
+    if (st != AERA_OK) return st;
+    cudaError_t e = cudaStreamSynchronize(s); // no kernel of an earlier call may still read the old weights
+    if (e != cudaSuccess) return cuda_fail(e, "stream synchronise");
+    if (!weights) { cudaFree(pl->d_filter); pl->d_filter = nullptr; pl->dev.bin_w = nullptr; return AERA_OK; }
+    if (n_weights != pl->dev.K)
+        return fail(AERA_ERR_INVALID_ARG, "n_weights=%d but the band of (n_samples=%d, fs=%g) has %d bins (aera_band)", n_weights, n_samples, fs_hz, pl->dev.K);
+    for (int j = 0; j < n_weights; ++j)
+        if (!std::isfinite(weights[j])) return fail(AERA_ERR_INVALID_ARG, "weights[%d] is not finite", j);
+    if (!pl->d_filter) {
+        e = cudaMalloc((void **)&pl->d_filter, sizeof(double) * pl->dev.K);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); pl->d_filter = nullptr; return fail(AERA_ERR_ALLOC, "cudaMalloc of the filter weights: %s", cudaGetErrorString(e)); }
+    }
+    e = cudaMemcpyAsync(pl->d_filter, weights, sizeof(double) * pl->dev.K, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "filter upload");
+    pl->dev.bin_w = pl->d_filter;
+    return AERA_OK;
 }
 
 size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,

@@ -91,7 +91,7 @@ __device__ inline DirCell direction_cell(const TableGeom &g, double theta, doubl
 template <typename T>
 __global__ void __launch_bounds__(128)
 minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restrict__ dirs,
-            const int *__restrict__ bin_if, const double *__restrict__ bin_tf, int K, double scale,
+            const int *__restrict__ bin_if, const double *__restrict__ bin_tf, const double *__restrict__ bin_w, int K, double scale0,
             int layout, int k_lo, int forward, cx<T> *__restrict__ minv)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -129,6 +129,7 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
 
     // per in-band bin: 1-D lerp in frequency, invert the 2x2 response, fold in 2/N
     for (int j = threadIdx.x; j < K; j += blockDim.x) {
+        const double scale = bin_w ? scale0 * bin_w[j] : scale0;   // pre-filter weight of this bin (aera_pattern_set_band_filter)
         const int jf = bin_if[j];
         const double t = bin_tf[j], t0 = 1.0 - t;
         double hr[4], hi[4];
@@ -191,12 +192,12 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
     if (dtype == AERA_F32) {
         e = cudaFuncSetAttribute(minv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf,
+        minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
                                                              p.K, scale, layout, p.k_lo, forward, (cx<float> *)minv);
     } else {
         e = cudaFuncSetAttribute(minv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf,
+        minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
                                                               p.K, scale, layout, p.k_lo, forward, (cx<double> *)minv);
     }
     count_launches(1);
