@@ -1,8 +1,8 @@
 """GPU parity of the device-resident reconstruction loop (aera_reconstruct_batch) against the loop oracle
-(oracle/aera_loop.py). Every step is checked on the GPU's own inputs of that step, so one admissible
-near-tie (a peak index off by one) cannot cascade into the later comparisons: where floating point decides
-an integer both sides must agree or be a near-tie; given the same integers and weights, the double-precision
-fit must agree to rounding."""
+(oracle/aera_loop.py). The oracle runs the whole loop on its own from the seeded inputs (nothing the CUDA
+path produced goes into it); every iteration's direction, peak amplitudes and peak indices and the final
+E-field traces are compared. An fp32 weight differs from the oracle's by ~2e-7 relative, which moves the
+fitted direction by < 1e-6 degree, far inside the tolerances of the unfolding itself."""
 import numpy as np
 import pytest
 import torch
@@ -43,27 +43,28 @@ def test_reconstruct_batch_step_by_step(B, cfg, n_events, n_st, n_iter):
     finally:
         pat.free()
     tie = TOL[wl.dtype]["tie"]
+    dir_tol = 1e-4 if wl.dtype == "f32" else 1e-9     # degrees
     for e in range(n_events):
+        o = ol.reconstruct_event(wl.grid, H, wl.fs_hz, tr[e], pos, n_iter)
         # timing from the voltages: exact unless the two maxima are a near-tie
-        o_idx0, o_w0 = ol.timing_from_voltages(tr[e])
         p = tr[e, :, 0, :].astype(np.float64) ** 2 + tr[e, :, 1, :].astype(np.float64) ** 2
         for s in range(n_st):
-            if g["idx0"][e, s] != o_idx0[s]:
-                assert 1.0 - p[s, g["idx0"][e, s]] / p[s, o_idx0[s]] < tie, (e, s)
-        assert np.allclose(g["w0"][e], o_w0, rtol=10 * TOL[wl.dtype]["amp"])
-        t, w = g["idx0"][e].astype(np.float64), g["w0"][e].astype(np.float64)
+            if g["idx0"][e, s] != o["idx0"][s]:
+                assert 1.0 - p[s, g["idx0"][e, s]] / p[s, o["idx0"][s]] < tie, (e, s)
+        assert np.allclose(g["w0"][e], o["w0"], rtol=10 * TOL[wl.dtype]["amp"])
         for it in range(n_iter):
-            th_o, ph_o = ol.planewave_fit(pos, t, w, wl.fs_hz)      # the oracle's fit on the GPU's integers / weights
+            th_o, ph_o = o["dirs"][it]
             th_g, ph_g = g["dirs_hist"][it, e]
-            assert abs(th_g - th_o) < 1e-8 and _ang(ph_g, ph_o) < 1e-8 / max(np.sin(np.deg2rad(th_o)), 1e-3), (e, it, th_g, th_o, ph_g, ph_o)
-            ref = oracle.unfold_batch(wl.grid, H, wl.fs_hz, tr[e], np.tile([th_g, ph_g], (n_st, 1)), want_env2=True)
+            assert abs(th_g - th_o) < dir_tol and _ang(ph_g, ph_o) < dir_tol / max(np.sin(np.deg2rad(th_o)), 1e-3), (e, it, th_g, th_o, ph_g, ph_o)
+            # peaks of this iteration against the oracle's own iteration (its direction, its unfolding)
+            ref = oracle.unfold_batch(wl.grid, H, wl.fs_hz, tr[e], np.tile(o["dirs"][it], (n_st, 1)), want_env2=True)
+            assert np.array_equal(ref["idx"], o["idx"][it])
             last = it == n_iter - 1
             rep = compare(wl.dtype, g["efield"][e] if last else None, g["amp_hist"][it, e], g["idx_hist"][it, e], ref)
             assert rep.ok(TOL[wl.dtype]), f"event {e} iteration {it}: {rep}"
-            t, w = g["idx_hist"][it, e].astype(np.float64), g["amp_hist"][it, e].astype(np.float64) ** 2
         # plausibility: the loop ends near the injected direction
-        th0, ph0 = evs[e].direction_deg
         # (in sin(theta): at large zenith angles a small error of the fitted (u, v) is a large one in theta)
+        th0, ph0 = evs[e].direction_deg
         assert abs(np.sin(np.deg2rad(g["dirs_hist"][-1, e, 0])) - np.sin(np.deg2rad(th0))) < 0.06, (e, g["dirs_hist"][:, e], th0, ph0)
 
 
