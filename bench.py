@@ -251,7 +251,7 @@ def run_loop(args, wl):
     true_dirs = np.stack([canon[e % n_canon].direction_deg for e in range(n_events)])
     d_tr = host.cuda(); d_pos = torch.from_numpy(pos).cuda()
     d_ef = torch.empty_like(d_tr)
-    ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_UNFOLD, pat, B.AERA_F32, n_events, wl.n_stations, wl.n_samples, wl.fs_hz))
+    ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_RECONSTRUCT, pat, B.AERA_F32, n_events, wl.n_stations, wl.n_samples, wl.fs_hz))
     stream = torch.cuda.current_stream()
     out = {}
 
@@ -279,9 +279,11 @@ def run_loop(args, wl):
     clocks = sampler.stop()
     n_units = n_events * wl.n_stations
     peak, peak_src = load_peaks()
-    # algorithmic bytes per unit and loop: the timing pass and every iteration read the 2 x N traces once; the last
-    # iteration also writes the E-field; 12 bytes of peaks per iteration
-    b_unit = 2 * wl.n_samples * 4 * (1 + n_iter) + 2 * wl.n_samples * 4 + 8 * (n_iter + 1)
+    # algorithmic bytes per unit and loop (spectrum reuse): the timing pass and the first iteration read
+    # the 2 x N traces; the first iteration writes the band spectra (19 rows x 32 x 16 B), every later one reads them;
+    # the last iteration writes the E-field; 8 bytes of peaks per iteration and for the voltage timing
+    spec = 19 * 32 * 16
+    b_unit = 2 * wl.n_samples * 4 * 2 + spec * (1 + max(n_iter - 1, 0) if n_iter > 1 else 0) + 2 * wl.n_samples * 4 + 8 * (n_iter + 1)
     achieved = n_units * b_unit / (ms_step * 1e-3) / 1e9
     dirs = out["r"]["dirs_hist"][-1].cpu().numpy()
     err = np.abs(np.sin(np.deg2rad(dirs[:, 0])) - np.sin(np.deg2rad(true_dirs[:, 0])))

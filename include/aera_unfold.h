@@ -92,7 +92,7 @@ aera_status_t aera_pattern_free(aera_pattern_t *pattern);
 aera_status_t aera_band(const aera_pattern_t *pattern, int n_samples, double fs_hz,
                         int *k_lo, int *k_hi);
 
-typedef enum { AERA_OP_UNFOLD = 0, AERA_OP_SCAN = 1, AERA_OP_FOLD = 2 } aera_op_t;
+typedef enum { AERA_OP_UNFOLD = 0, AERA_OP_SCAN = 1, AERA_OP_FOLD = 2, AERA_OP_RECONSTRUCT = 3 } aera_op_t;
 
 /* Scratch bytes needed by aera_unfold_batch (n_events_or_dirs = n_events) or
  * aera_scan_directions (n_events_or_dirs = n_dirs) for these sizes; 0 on invalid arguments
@@ -188,7 +188,10 @@ aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_ev
  *   efield    as in aera_unfold_batch; may be NULL; may alias traces (written in the last iteration only)
  *   amp_hist  [n_iter][n_events][n_stations] real (dtype), idx_hist the same shape int32     device, out
  *   idx0 / w0 [n_events][n_stations] int32 / real (dtype): the voltage timing                 device, out
- *   workspace as for aera_unfold_batch (AERA_OP_UNFOLD size for n_events)
+ *   workspace >= aera_workspace_bytes(AERA_OP_UNFOLD, ...) for n_events. With
+ *             aera_workspace_bytes(AERA_OP_RECONSTRUCT, ...) or more (room for the direction-independent band
+ *             spectra of every station, 9.7 KB each at configs[1]) the first iteration stores them and the later
+ *             ones start from them: no trace re-read, no forward transform (results are bit-identical)
  * Asynchronous on the stream; errors as aera_unfold_batch, plus AERA_ERR_INVALID_ARG for n_iter < 1.
  */
 aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,

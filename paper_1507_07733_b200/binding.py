@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 AERA_F32, AERA_F64 = 0, 1
-AERA_OP_UNFOLD, AERA_OP_SCAN, AERA_OP_FOLD = 0, 1, 2
+AERA_OP_UNFOLD, AERA_OP_SCAN, AERA_OP_FOLD, AERA_OP_RECONSTRUCT = 0, 1, 2, 3
 STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 3: "AERA_ERR_DTYPE_MISMATCH",
           4: "AERA_ERR_WORKSPACE", 5: "AERA_ERR_ALLOC", 6: "AERA_ERR_CUDA", 7: "AERA_ERR_BAND"}
 
@@ -284,7 +284,7 @@ def aera_reconstruct_batch(p: Pattern, traces: torch.Tensor, positions: torch.Te
     idx0 = torch.empty((E, S), dtype=torch.int32, device=dev)
     w0 = torch.empty((E, S), dtype=traces.dtype, device=dev)
     if workspace is None:
-        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, dev)
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_RECONSTRUCT, p, dt, E, S, N, fs_hz) if E > 0 else 256, dev)
     _check(_lib.aera_reconstruct_batch(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(positions), n_iter, _ptr(dirs_hist),
                                        _ptr(efield) if efield is not None else None, _ptr(amp_hist), _ptr(idx_hist), _ptr(idx0), _ptr(w0),
                                        _ptr(workspace), workspace.numel(), _stream_ptr(stream)))

@@ -74,8 +74,11 @@ cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, con
 
 // ---- unfold_w32.cu: warp-per-station kernel for N = 2048 fp32 with the band below N/2
 bool w32_supported(int dtype, const PlanDev &p);
+// spectra / spec_mode: 1 = also store the direction-independent band spectra 2 V_c, 2 = start from them (no trace
+// read, no forward transform); w32_spectra_bytes() = 0 when the band geometry has no such instantiation
+size_t w32_spectra_bytes(const PlanDev &p, long n_units);
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                              void *amp, int32_t *idx, const void *minv, cudaStream_t s);
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra = nullptr, int spec_mode = 0);
 
 // ---- unfold_t4k_f64.cu: team-per-station kernel for N = 4096 fp64, band rows 4..12 (configs[3])
 bool t4k_f64_supported(int dtype, const PlanDev &p);

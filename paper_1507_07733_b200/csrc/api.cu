@@ -231,7 +231,7 @@ TableGeom geom_of(const aera_pattern_desc_t &d)
 }
 
 struct WsLayout {
-    size_t off_minv, off_scratch, off_spectra, off_peaks, total;
+    size_t off_minv, off_scratch, off_spectra, off_loop_spectra, off_peaks, total;
 };
 
 // Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
@@ -255,6 +255,9 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
         size_t a = generic_scan_spectra_bytes(dtype, K, n_stations), b = scan_w32_spectra_bytes(n_stations);
         o = align_up(o + (a > b ? a : b));
     }
+    w.off_loop_spectra = o;                                               // reconstruction loop: band spectra of every station
+    if (op == AERA_OP_RECONSTRUCT && dtype == AERA_F32 && w32_supported(dtype, band))
+        o = align_up(o + w32_spectra_bytes(band, n_dirs * (long)n_stations));
     w.off_peaks = o;                                                      // fold: the by-product peaks of the shared kernels
     if (op == AERA_OP_FOLD) o = align_up(o + (size_t)n_dirs * n_stations * 12);
     w.total = o > 0 ? o : kAlign;
@@ -406,7 +409,7 @@ aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_sample
 size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,
                             int n_stations, int n_samples, double fs_hz)
 {
-    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN && op != AERA_OP_FOLD) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
+    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN && op != AERA_OP_FOLD && op != AERA_OP_RECONSTRUCT) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
     if (check_common(pattern, dtype, n_stations, n_samples, fs_hz) != AERA_OK) return 0;
     if (n_events_or_dirs < 0) { fail(AERA_ERR_INVALID_ARG, "negative count"); return 0; }
     int k_lo, k_hi;
@@ -419,7 +422,7 @@ size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dty
 static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
                                  int n_samples, double fs_hz, const void *traces, const double *dirs,
                                  void *efield, void *peak_amp, int32_t *peak_idx,
-                                 void *workspace, size_t workspace_bytes, void *cuda_stream, int forward)
+                                 void *workspace, size_t workspace_bytes, void *cuda_stream, int forward, int spec_mode = 0)
 {
     aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
     if (st != AERA_OK) return st;
@@ -434,7 +437,8 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     Plan *pl = nullptr;
     st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
     if (st != AERA_OK) return st;
-    const WsLayout w = ws_layout(forward ? AERA_OP_FOLD : AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, n_events, n_stations);
+    const WsLayout w = ws_layout(forward ? AERA_OP_FOLD : (spec_mode ? AERA_OP_RECONSTRUCT : AERA_OP_UNFOLD), dtype, n_samples,
+                                 pl->dev.k_lo, pl->dev.K, n_events, n_stations);
     if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
@@ -452,7 +456,8 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
                                 ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s, forward);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     if (warp_path)
-        e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
+        e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s,
+                              spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode);
     else if (team_path)
         e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
     else if (long_path)
@@ -539,6 +544,16 @@ aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, i
     const size_t units = (size_t)n_events * n_stations;
     cudaError_t e = launch_timing(dtype, traces, (long)units, n_samples, idx0, w0, s);
     if (e != cudaSuccess) return cuda_fail(e, "timing kernel launch");
+    // spectrum reuse (fp32 warp kernel only): needs the larger AERA_OP_RECONSTRUCT workspace
+    bool reuse = false;
+    if (n_iter > 1 && kernel_variant() == 0 && dtype == AERA_F32) {
+        int k_lo, k_hi;
+        if (compute_band(pattern->desc, n_samples, fs_hz, &k_lo, &k_hi) == AERA_OK) {
+            PlanDev band{}; band.N = n_samples; band.k_lo = k_lo; band.k_hi = k_hi; band.K = k_hi - k_lo + 1;
+            reuse = w32_supported(dtype, band) && w32_spectra_bytes(band, (long)units) > 0 &&
+                    workspace_bytes >= ws_layout(AERA_OP_RECONSTRUCT, dtype, n_samples, k_lo, band.K, n_events, n_stations).total;
+        }
+    }
     const int32_t *t_idx = idx0;
     const void *t_w = w0;
     int square = 0;
@@ -548,8 +563,9 @@ aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, i
         if (e != cudaSuccess) return cuda_fail(e, "plane-wave fit kernel launch");
         void *amp = static_cast<unsigned char *>(amp_hist) + (size_t)it * units * rb;
         int32_t *idx = idx_hist + (size_t)it * units;
-        st = aera_unfold_batch(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs,
-                               it == n_iter - 1 ? efield : nullptr, amp, idx, workspace, workspace_bytes, cuda_stream);
+        st = unfold_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs,
+                         it == n_iter - 1 ? efield : nullptr, amp, idx, workspace, workspace_bytes, cuda_stream, 0,
+                         reuse ? (it == 0 ? 1 : 2) : 0);
         if (st != AERA_OK) return st;
         t_idx = idx; t_w = amp; square = 1;
     }

@@ -47,6 +47,7 @@ struct W32Params {
     float *amp;
     int32_t *idx;
     const float4 *minv;   // [n_events] { A[K], B[K] } float4, see MINV_PACKED
+    float4 *spectra;      // [n_units][band rows][32] {2V0.re, 2V0.im, 2V1.re, 2V1.im}: written (SPEC 1) or read (SPEC 2)
     const float2 *tw1024; // W_1024^m
     const float2 *twN;    // W_2048^m
     long n_units;
@@ -58,9 +59,11 @@ struct W32Params {
 // spectrum G_r (r = 0, 1 in the two halves). Separates the channels with the mirror bin 1024-k,
 // folds the two polyphase halves (2 V_c = F'_c0 + W_2048^k F'_c1), applies Minv (a4) and leaves
 // (E_theta, E_phi) packed as (re, im) in tensor-memory columns 4r .. 4r+3 of this lane.
-template <class G, bool MINV_SMEM>
+// SPEC = 1 also stores 2 V_c of the band rows (direction-independent: later iterations of the reconstruction loop
+// start from them, SPEC = 2, and skip the trace read and the forward transform).
+template <class G, bool MINV_SMEM, int SPEC>
 __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const float2 *TS, const float4 *MA,
-                                               const float4 *MB, int k_lo, int k_hi, int lane, uint32_t tstash)
+                                               const float4 *MB, int k_lo, int k_hi, int lane, uint32_t tstash, float4 *sp)
 {
     // partner bin 1024-k lives in lane (32-lane)&31, row 31-k2 (row 32-k2 for lane 0)
     // (k = 0, whose partner row would be 32, is never in band: k_lo >= 1)
@@ -70,6 +73,7 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
 #pragma unroll 1
     for (int r = 0; r < G::kBandRows; ++r, own += 32, par -= 32, k += 32) {
         R er = L::zero(), ei = L::zero();
+        float4 vsp = make_float4(0.f, 0.f, 0.f, 0.f);
         if (k >= k_lo && k <= k_hi) {
             const R ar = QA[own], ai = QB[own], pr = QA[par], pi = QB[par];
             // F'_0 = G + conj(Gm) = 2 FFT(v0 polyphase r), F'_1 = -i (G - conj(Gm)) = 2 FFT(v1 polyphase r)
@@ -83,6 +87,7 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
             float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
             float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
             float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
+            if (SPEC == 1) vsp = make_float4(v0r, v0i, v1r, v1i);
             const float4 m0 = MINV_SMEM ? MA[k - k_lo] : ld_nc_f4(MA + (k - k_lo));
             const float4 m1 = MINV_SMEM ? MB[k - k_lo] : ld_nc_f4(MB + (k - k_lo));
             const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
@@ -91,12 +96,46 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
             ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
             ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
         }
+        if (SPEC == 1) sp[r * 32] = vsp;
         tmem_st64(tstash + 4 * r, er.v);
         tmem_st64(tstash + 4 * r + 2, ei.v);
     }
 }
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, bool TIGHT>
+// SPEC = 2: a4 straight from the stored 2 V_c of this station (zero outside the band).
+// The rows are first copied to the warp's shared-memory buffer with independent loads (one latency, not one
+// per row of the rolled loop).
+template <class G, bool MINV_SMEM>
+__device__ __forceinline__ void solve_from_spectra(const float4 *sp, float4 *XV, const float4 *MA, const float4 *MB, int k_lo,
+                                                   int k_hi, int lane, uint32_t tstash)
+{
+    static_assert(G::kBandRows * 512 <= G::kWarpBytes, "band rows fit the warp buffer");
+    {
+        float4 tmp[G::kBandRows];
+        static_for<0, G::kBandRows>([&](auto rc) { constexpr int r = decltype(rc)::value; tmp[r] = ld_nc_f4(sp + r * 32); });
+        static_for<0, G::kBandRows>([&](auto rc) { constexpr int r = decltype(rc)::value; XV[r * 32 + lane] = tmp[r]; });
+    }
+    __syncwarp();
+    int k = lane + 32 * G::kLo;
+#pragma unroll 1
+    for (int r = 0; r < G::kBandRows; ++r, k += 32) {
+        R er = L::zero(), ei = L::zero();
+        if (k >= k_lo && k <= k_hi) {
+            const float4 v = XV[r * 32 + lane];
+            const float4 m0 = MINV_SMEM ? MA[k - k_lo] : ld_nc_f4(MA + (k - k_lo));
+            const float4 m1 = MINV_SMEM ? MB[k - k_lo] : ld_nc_f4(MB + (k - k_lo));
+            const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
+            er = L::mul(Ma, L::bc(v.x)); er = L::fma(Mb, L::bc(-v.y), er);
+            er = L::fma(Mc, L::bc(v.z), er); er = L::fma(Md, L::bc(-v.w), er);
+            ei = L::mul(Ma, L::bc(v.y)); ei = L::fma(Mb, L::bc(v.x), ei);
+            ei = L::fma(Mc, L::bc(v.w), ei); ei = L::fma(Md, L::bc(v.z), ei);
+        }
+        tmem_st64(tstash + 4 * r, er.v);
+        tmem_st64(tstash + 4 * r + 2, ei.v);
+    }
+}
+
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC>
 __global__ void __launch_bounds__(W32Geom<K2LO, K2HI>::kWarps * 32, 1)
 unfold_w32_kernel(W32Params p)
 {
@@ -163,15 +202,28 @@ unfold_w32_kernel(W32Params p)
         for (long u = first; u < hi; u += kWarps) {
             const float *v = p.traces + (size_t)u * 4 * kM;
             float *ef = HAS_EF ? p.efield + (size_t)u * 4 * kM : nullptr;
-            if (lane == 0 && u + kWarps < u1) prefetch_l2_bulk(v + (size_t)kWarps * 4 * kM, 4 * kM * sizeof(float));
+            float4 *sp = SPEC != 0 ? p.spectra + (size_t)u * G::kBandRows * 32 + lane : nullptr;
+            if (lane == 0 && u + kWarps < u1) {
+                if (SPEC != 2) prefetch_l2_bulk(v + (size_t)kWarps * 4 * kM, 4 * kM * sizeof(float));
+                else prefetch_l2_bulk(p.spectra + (size_t)(u + kWarps) * G::kBandRows * 32, G::kBandRows * 32 * sizeof(float4));
+            }
 
-            // ---- a1: the station's two traces, read once, straight into FFT input order
             R A[32], B[32];
-            static_for<0, 32>([&](auto jc) {
-                constexpr int j = decltype(jc)::value;
-                A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
-                B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
-            });
+            if constexpr (SPEC != 2) {
+                // ---- a1: the station's two traces, read once, straight into FFT input order
+                static_for<0, 32>([&](auto jc) {
+                    constexpr int j = decltype(jc)::value;
+                    A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
+                    B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
+                });
+            } else {
+                // ---- the forward spectrum of this station was stored by an earlier call: a4 straight away
+                if (!minv_ready) { mbar_wait(&full[slot], parity); minv_ready = true; }
+                solve_from_spectra<G, MINV_SMEM>(sp, reinterpret_cast<float4 *>(X), MA, MB, p.k_lo, p.k_hi, lane, tstash);
+                __syncwarp(); // the buffer becomes a transpose plane again
+                tmem_wait_st();
+                build_inverse_input<G, false>(B, A, TS, lane, tstash);
+            }
 
             // ---- three 1024-point transforms through ONE copy of the FFT code (the instruction
             // stream of a fully unrolled station is ~90 KB, far beyond the instruction caches; with
@@ -181,7 +233,7 @@ unfold_w32_kernel(W32Params p)
             float best0 = -1.0f, best1 = -1.0f; int b0 = 0, b1 = 0;
             // (Loops are written so that each exit leaves straight from the FFT: a join of the
             // "continue" and "exit" paths would cost a register shuffle on every pass.)
-            int t = 0;
+            int t = SPEC == 2 ? 1 : 0;
 #pragma unroll 1
             for (;;) {
                 int second = 0;
@@ -197,7 +249,7 @@ unfold_w32_kernel(W32Params p)
                     asm volatile("" : "+r"(second));
                 }
                 if (t == 2) break;
-                if (t == 0) {
+                if (SPEC != 2 && t == 0) {
                     // ---- a2 done: publish the band rows and the rows that are somebody's bin 1024-k
                     static_for<G::kPubLo, G::kPubHi + 1>([&](auto rc) {
                         constexpr int r = decltype(rc)::value;
@@ -209,7 +261,7 @@ unfold_w32_kernel(W32Params p)
                     // ---- separate channels, fold the two polyphase halves, a4: E = Minv V, one band
                     // row per iteration (a rolled loop: 40 instructions instead of 19 x 45), E goes to
                     // this lane's tensor-memory columns and is read back twice (s = 0, 1)
-                    separate_solve<G, MINV_SMEM>(QA, QB, TS, MA, MB, p.k_lo, p.k_hi, lane, tstash);
+                    separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MA, MB, p.k_lo, p.k_hi, lane, tstash, sp);
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
                     // ---- a5: even samples  z[2m] = IFFT_1024(E): inverse roles, A = Im, B = Re
@@ -272,12 +324,12 @@ size_t w32_smem_bytes(int K)
     return (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)G::kWarps * G::kWarpBytes;
 }
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, bool TIGHT>
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC>
 cudaError_t launch_inst(const W32Params &q, cudaStream_t s)
 {
     using G = W32Geom<K2LO, K2HI>;
     const size_t smem = w32_smem_bytes<K2LO, K2HI, MINV_SMEM>(q.K);
-    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, TIGHT>;
+    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, SPEC>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     long grid = (q.n_units + G::kWarps - 1) / G::kWarps;
@@ -293,21 +345,31 @@ bool w32_supported(int dtype, const PlanDev &p)
     return dtype == AERA_F32 && p.N == 2 * kM && p.k_hi < kM && p.k_lo >= 1;
 }
 
+size_t w32_spectra_bytes(const PlanDev &p, long n_units)
+{
+    // only the configs[1] band geometry has the spectrum-reuse instantiations
+    if (!((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28)) return 0;
+    return (size_t)n_units * W32Geom<10, 28>::kBandRows * 32 * sizeof(float4);
+}
+
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                              void *amp, int32_t *idx, const void *minv, cudaStream_t s)
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra, int spec_mode)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
     ProfScope prof(KID_UNFOLD, s);
     W32Params q;
     q.traces = (const float *)traces; q.efield = (float *)efield; q.amp = (float *)amp; q.idx = idx;
+    q.spectra = (float4 *)spectra;
     q.minv = (const float4 *)minv; q.tw1024 = (const float2 *)p.tw1024; q.twN = (const float2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     cudaError_t e;
-    if ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) // configs[1]: 30-80 MHz at fs = 180 MHz
-        e = efield ? launch_inst<10, 28, true, true, true>(q, s) : launch_inst<10, 28, false, true, true>(q, s);
-    else
-        e = efield ? launch_inst<0, 31, true, false, false>(q, s) : launch_inst<0, 31, false, false, false>(q, s);
+    if ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) { // configs[1]: 30-80 MHz at fs = 180 MHz
+        if (spectra && spec_mode == 1) e = efield ? launch_inst<10, 28, true, true, 1>(q, s) : launch_inst<10, 28, false, true, 1>(q, s);
+        else if (spectra && spec_mode == 2) e = efield ? launch_inst<10, 28, true, true, 2>(q, s) : launch_inst<10, 28, false, true, 2>(q, s);
+        else e = efield ? launch_inst<10, 28, true, true, 0>(q, s) : launch_inst<10, 28, false, true, 0>(q, s);
+    } else
+        e = efield ? launch_inst<0, 31, true, false, 0>(q, s) : launch_inst<0, 31, false, false, 0>(q, s);
     count_launches(1);
     return e;
 }

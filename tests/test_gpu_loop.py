@@ -88,3 +88,25 @@ def test_reconstruct_batch_errors_and_inplace(B):
         assert torch.equal(c["efield"], a["efield"]) and torch.equal(c["amp_hist"], a["amp_hist"])
     finally:
         pat.free()
+
+
+def test_spectrum_reuse_is_bit_identical(B):
+    """With the larger AERA_OP_RECONSTRUCT workspace the first iteration stores the direction-independent band
+    spectra and the later ones start from them (no trace re-read, no forward transform): same bits out."""
+    wl = ai.WORKLOADS[1]
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    pos = ai.station_positions(31)
+    tr = np.stack([ai.make_event(wl, e, n_stations=31, positions=pos).traces for e in range(3)])
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        d_tr = torch.from_numpy(tr).cuda(); d_pos = torch.from_numpy(pos).cuda()
+        small = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_UNFOLD, pat, B.AERA_F32, 3, 31, wl.n_samples, wl.fs_hz))
+        big = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_RECONSTRUCT, pat, B.AERA_F32, 3, 31, wl.n_samples, wl.fs_hz))
+        assert big.numel() > small.numel()
+        a = B.aera_reconstruct_batch(pat, d_tr, d_pos, wl.fs_hz, 3, workspace=small)
+        b = B.aera_reconstruct_batch(pat, d_tr, d_pos, wl.fs_hz, 3, workspace=big)
+        torch.cuda.synchronize()
+        for k in ("dirs_hist", "efield", "amp_hist", "idx_hist", "idx0", "w0"):
+            assert torch.equal(a[k], b[k]), k
+    finally:
+        pat.free()
