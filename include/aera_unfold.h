@@ -166,10 +166,12 @@ aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_ev
                               void *traces, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
- * Device-resident reconstruction loop (section 2, L29 and Fig. 1: "the maxima of the voltage
- * traces are used as an initial guess on the signal timing and the direction is reconstructed from
- * triangulation [...] the E-field trace at each station reconstructed [...] the maximum of the envelope
- * [...] is used as updated timing information, and the process is iterated"; section 5, L83 names keeping
+ * Device-resident reconstruction loop (section 2, L29 and Fig. 1: "First, as an initial estimate of the
+ * event timing in each station, the maxima of the voltage traces is used. Second, from the timing information of
+ * the individual stations, the direction of the shower is obtained by triangulation. Third, the antenna pattern
+ * for this direction is evaluated, and the E-field trace at each station reconstructed from the voltage traces.
+ * Finally, the maximum of the envelope of the E-field trace is used as updated timing information for a new
+ * iteration of the procedure."; section 5, L83 names keeping
  * the data on the GPU as the remedy for copy-dominated run time). Per event, all on the device:
  *
  *   n_i, w_i = lowest n maximising v0[n]^2 + v1[n]^2 and that maximum          (timing from the voltages)

@@ -1,8 +1,9 @@
 """Oracle of the device-resident reconstruction loop (SURVEY.md 8f "next" row 1; Fig. 1:
-"the maxima of the voltage traces are used as an initial guess on the signal timing and the direction
-is reconstructed from triangulation. [...] the E-field trace at each station reconstructed [...] the
-maximum of the envelope of the E-field trace is used as updated timing information, and the process is
-iterated"; L83 names keeping the data on the GPU as the remedy for copy-dominated run time).
+"First, as an initial estimate of the event timing in each station, the maxima of the voltage traces is
+used. Second, from the timing information of the individual stations, the direction of the shower is obtained
+by triangulation. Third, the antenna pattern for this direction is evaluated, and the E-field trace at each
+station reconstructed from the voltage traces. Finally, the maximum of the envelope of the E-field trace is
+used as updated timing information for a new iteration of the procedure."; L83 names keeping the data on the GPU as the remedy for copy-dominated run time).
 
 TEST INFRASTRUCTURE ONLY (see oracle/__init__.py): plain numpy in float64, one step per function, in
 the paper's order. The per-station unfolding inside the loop is oracle.unfold_batch (aera_oracle.c).

@@ -361,9 +361,12 @@ long oracle_unfold_station_spectra(const oracle_grid_t *g, const double *H, int 
 }
 
 /* Direction scan (BASELINE configs[2]): O1 once per station, O3-O7 for every direction.
- * traces [S][2][N]; dirs [D][2]; amp, idx [D][S].  OpenMP over (direction, station). */
+ * traces [S][2][N]; dirs [D][2]; amp, idx [D][S]; env2 [D][S][N] or NULL (the squared envelope
+ * of every pair, so that a test can apply the near-tie rule of BASELINE north_star: "+-1 allowed when
+ * the top two envelope values differ by < 1e-5 relative").  OpenMP over (direction, station). */
 long oracle_scan(const oracle_grid_t *g, const double *H, int S, int N, double fs_hz,
-                 const double *traces, long D, const double *dirs, double *amp, int32_t *idx)
+                 const double *traces, long D, const double *dirs, double *amp, int32_t *idx,
+                 double *env2)
 {
     long k_lo, k_hi;
     oracle_band(N, fs_hz, g->n_freq, g->freq0_hz, g->dfreq_hz, &k_lo, &k_hi);
@@ -401,7 +404,7 @@ long oracle_scan(const oracle_grid_t *g, const double *H, int S, int N, double f
             oracle_analytic_from_band(Etr, Eti, N, k_lo, k_hi, Wre, Wim, ztr, zti);
             oracle_analytic_from_band(Epr, Epi, N, k_lo, k_hi, Wre, Wim, zpr, zpi);
         }
-        oracle_peak(ztr, zti, zpr, zpi, N, NULL, amp + p, idx + p);
+        oracle_peak(ztr, zti, zpr, zpi, N, env2 ? env2 + (size_t)p * N : NULL, amp + p, idx + p);
         free(w);
     }
     free(V); free(Wre); free(Wim);

@@ -159,18 +159,19 @@ def unfold_station_spectra(grid, H, fs_hz: float, v, theta_deg: float, phi_deg: 
                 V0=sp[0], V1=sp[1], Et=sp[2], Ep=sp[3])
 
 
-def scan(grid, H, fs_hz: float, traces, dirs):
-    """traces [S][2][N], dirs [D][2] -> amp [D][S], idx [D][S] int32."""
+def scan(grid, H, fs_hz: float, traces, dirs, want_env2=False):
+    """traces [S][2][N], dirs [D][2] -> amp [D][S], idx [D][S] int32 (and env2 [D][S][N] with want_env2)."""
     H = _table(grid, H)
     tr = np.ascontiguousarray(traces, dtype=np.float64)
     S, two, N = tr.shape
     dd = np.ascontiguousarray(dirs, dtype=np.float64)
     D = dd.shape[0]
     amp = np.empty((D, S)); idx = np.empty((D, S), dtype=np.int32)
+    e2 = np.empty((D, S, N)) if want_env2 else None
     g = _grid(grid)
     _lib.oracle_scan(C.byref(g), _d(H.view(np.float64)), C.c_int(S), C.c_int(N), C.c_double(fs_hz),
-                     _d(tr), C.c_long(D), _d(dd), _d(amp), idx.ctypes.data_as(_ip))
-    return amp, idx
+                     _d(tr), C.c_long(D), _d(dd), _d(amp), idx.ctypes.data_as(_ip), _d(e2))
+    return (amp, idx, e2) if want_env2 else (amp, idx)
 
 
 def fold_station(grid, H, N: int, fs_hz: float, Et, Ep, theta_deg: float, phi_deg: float):

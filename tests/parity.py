@@ -50,40 +50,63 @@ def compare(dtype: str, gpu_efield, gpu_amp, gpu_idx, orc: dict) -> Report:
         da = abs(float(gpu_amp[u]) - orc["amp"][u]) / orc["amp"][u]
         rep.max_amp = max(rep.max_amp, da)
         io, ig = int(orc["idx"][u]), int(gpu_idx[u])
-        if ig == io:
+        kind, gap = classify_index(tol, io, ig, orc["env2"][u])
+        if kind == "exact":
             rep.idx_exact += 1
+        elif kind == "tie":
+            rep.idx_tie_pm1 += 1
         else:
-            e2 = orc["env2"][u]
-            N = len(e2)
-            gap = 1.0 - np.sqrt(e2[ig] / e2[io]) if 0 <= ig < N else 1.0
-            if gap < tol["tie"] and abs(ig - io) <= 1:
-                rep.idx_tie_pm1 += 1
-            elif gap < tol["tie"]:
+            if kind == "ambiguous":
                 rep.idx_ambiguous += 1
-                rep.bad.append((u, io, ig, float(gap)))
             else:
                 rep.idx_miss += 1
-                rep.bad.append((u, io, ig, float(gap)))
+            rep.bad.append((u, io, ig, float(gap)))
     if l2s:
         rep.max_l2 = float(np.max(l2s))
         rep.med_l2 = float(np.median(l2s))
     return rep
 
 
-def compare_peaks(dtype: str, gpu_amp, gpu_idx, orc_amp, orc_idx, tie_env2=None) -> Report:
-    """Peaks only (scan mode): amp relative error and exact index (near-ties need env2, not available here)."""
+def classify_index(tol, io: int, ig: int, e2) -> tuple[str, float]:
+    """BASELINE north_star rule for one unit: exact, or +-1 when the oracle envelope at the GPU's index is
+    within tol["tie"] (relative) of the oracle maximum; a near-tie further away is "ambiguous" (counted as a
+    miss by Report.ok), anything else a miss. e2 = the ORACLE's squared envelope of the unit."""
+    if ig == io:
+        return "exact", 0.0
+    N = len(e2)
+    gap = 1.0 - float(np.sqrt(e2[ig] / e2[io])) if 0 <= ig < N else 1.0
+    if gap < tol["tie"] and abs(ig - io) <= 1:
+        return "tie", gap
+    return ("ambiguous" if gap < tol["tie"] else "miss"), gap
+
+
+def compare_peaks(dtype: str, gpu_amp, gpu_idx, orc_amp, orc_idx, orc_env2) -> Report:
+    """Peaks only (scan mode). orc_env2 [..][N] is the oracle's squared envelope of every compared pair
+    (oracle.scan(..., want_env2=True)), so the index rule is the stated one, not a proxy."""
     tol = TOL[dtype]
     ga = np.asarray(gpu_amp, dtype=np.float64).ravel(); gi = np.asarray(gpu_idx).ravel()
     oa = np.asarray(orc_amp).ravel(); oi = np.asarray(orc_idx).ravel()
+    e2 = np.asarray(orc_env2).reshape(len(oa), -1)
     rep = Report(n=len(oa))
     rep.max_amp = float(np.max(np.abs(ga - oa) / oa))
-    rep.idx_exact = int(np.sum(gi == oi))
-    mism = np.nonzero(gi != oi)[0]
-    for m in mism:
-        # without env2 the only admissible mismatch is +-1 with amplitudes equal to within the tie window
-        if abs(int(gi[m]) - int(oi[m])) <= 1 and abs(ga[m] - oa[m]) / oa[m] < tol["tie"] * 10:
+    for m in range(len(oa)):
+        kind, gap = classify_index(tol, int(oi[m]), int(gi[m]), e2[m])
+        if kind == "exact":
+            rep.idx_exact += 1
+        elif kind == "tie":
             rep.idx_tie_pm1 += 1
         else:
-            rep.idx_miss += 1
-            rep.bad.append((int(m), int(oi[m]), int(gi[m])))
+            if kind == "ambiguous":
+                rep.idx_ambiguous += 1
+            else:
+                rep.idx_miss += 1
+            rep.bad.append((int(m), int(oi[m]), int(gi[m]), gap))
     return rep
+
+
+def assert_peaks(rep: Report, dtype: str, max_ties: int = 0):
+    """Scan-mode verdict: amplitude bound, no miss / ambiguous maximum, and at most `max_ties` +-1 near-ties
+    (0 on the seeded inputs of this repository: a systematic off-by-one would show up here)."""
+    tol = TOL[dtype]
+    assert rep.max_amp <= tol["amp"] and rep.idx_miss == 0 and rep.idx_ambiguous == 0, str(rep)
+    assert rep.idx_tie_pm1 <= max_ties, f"{rep.idx_tie_pm1} near-tie +-1 index mismatches (allowed {max_ties}): {rep}"

@@ -6,7 +6,7 @@ import pytest
 import torch
 
 import aera_inputs as ai
-from parity import TOL, compare, compare_peaks
+from parity import TOL, assert_peaks, compare, compare_peaks
 
 pytestmark = pytest.mark.gpu
 
@@ -75,8 +75,9 @@ def test_filtered_scan_matches_oracle(B):
     finally:
         pat.free()
     oamp = np.empty((len(dirs), len(tr))); oidx = np.empty((len(dirs), len(tr)), dtype=np.int32)
+    oe2 = np.empty((len(dirs), len(tr), wl.n_samples))
     for d in range(len(dirs)):
         r = of.unfold_batch_filtered(wl.grid, H, wl.fs_hz, tr, np.tile(dirs[d], (len(tr), 1)), w)
-        oamp[d] = r["amp"]; oidx[d] = r["idx"]
-    rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx)
-    assert rep.max_amp <= TOL["f32"]["amp"] and rep.idx_miss == 0, str(rep)
+        oamp[d] = r["amp"]; oidx[d] = r["idx"]; oe2[d] = r["env2"]
+    rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx, oe2)
+    assert_peaks(rep, wl.dtype)

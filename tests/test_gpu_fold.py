@@ -18,7 +18,7 @@ def B():
     return b
 
 
-@pytest.mark.parametrize("cfg,n_events,n_st,variant", [(0, 2, 7, 0), (1, 2, 9, 0), (1, 1, 5, 1), (3, 2, 5, 0)])
+@pytest.mark.parametrize("cfg,n_events,n_st,variant", [(0, 2, 7, 0), (1, 2, 9, 0), (1, 1, 5, 1), (3, 2, 5, 0), (4, 1, 2, 0)])
 def test_fold_matches_oracle_and_round_trips(B, cfg, n_events, n_st, variant):
     import oracle
     wl = ai.WORKLOADS[cfg]

@@ -24,7 +24,7 @@ def _ang(a, b):
     return abs((a - b + 180.0) % 360.0 - 180.0)
 
 
-@pytest.mark.parametrize("cfg,n_events,n_st,n_iter", [(1, 5, 124, 3), (0, 2, 7, 2), (3, 3, 40, 2)])
+@pytest.mark.parametrize("cfg,n_events,n_st,n_iter", [(1, 5, 124, 3), (0, 2, 7, 2), (3, 3, 40, 2), (4, 1, 8, 2)])
 def test_reconstruct_batch_step_by_step(B, cfg, n_events, n_st, n_iter):
     import oracle
     from oracle import aera_loop as ol

@@ -276,6 +276,14 @@ def test_scan_equals_batch_per_direction(small_grid, small_table):
         r = oracle.unfold_batch(g, H, wl.fs_hz, ev.traces, np.repeat(dirs[d][None], wl.n_stations, axis=0))
         assert np.array_equal(idx[d], r["idx"])
         assert np.max(np.abs(amp[d] - r["amp"])) <= 1e-13 * np.max(r["amp"])
+    # the optional squared-envelope output (used by the scan parity tests for the near-tie rule) is the batch
+    # oracle's env2 and is consistent with the returned peaks
+    amp2, idx2, e2 = oracle.scan(g, H, wl.fs_hz, ev.traces, dirs, want_env2=True)
+    assert np.array_equal(amp2, amp) and np.array_equal(idx2, idx) and e2.shape == (len(dirs), wl.n_stations, wl.n_samples)
+    for d in range(len(dirs)):
+        r = oracle.unfold_batch(g, H, wl.fs_hz, ev.traces, np.repeat(dirs[d][None], wl.n_stations, axis=0), want_env2=True)
+        assert np.max(np.abs(e2[d] - r["env2"])) <= 1e-12 * np.max(r["env2"])
+    assert np.array_equal(np.argmax(e2, axis=-1), idx) and np.array_equal(np.sqrt(np.max(e2, axis=-1)), amp)
 
 
 # ---------------------------------------------------------------- generator sanity (no method arithmetic)
