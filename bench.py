@@ -171,6 +171,36 @@ def run_reference(args, wl):
     print(json.dumps(line), flush=True)
 
 
+def measure_alu_peaks(B):
+    """Measured FMA issue peaks of this device (aera_measure_alu_peak: register-only FMA chains on every SM, CUDA
+    events, best over 4..32 warps per SM): packed fp32 (FFMA2, the warp kernels' instruction), scalar fp32, fp64."""
+    out = {}
+    for name, kind in B.ALU_KINDS.items():
+        best = None
+        for w in (4, 8, 16, 32):
+            r = B.aera_measure_alu_peak(kind, w)
+            if best is None or r["lane_fma_per_s"] > best["lane_fma_per_s"]:
+                best = dict(r, warps_per_sm=w)
+        clk = best["sm_clock_khz"] * 1e3
+        out[name] = {"tflops": 2 * best["lane_fma_per_s"] / 1e12, "lane_fma_per_s": best["lane_fma_per_s"],
+                     "lane_fma_per_clk_per_sm": best["lane_fma_per_s"] / best["sm_count"] / clk, "warps_per_sm": best["warps_per_sm"],
+                     "sm_count": best["sm_count"], "sm_clock_mhz": clk / 1e6}
+    return out
+
+
+def run_peaks(args):
+    """--peaks: print the measured ALU peaks (one JSON line); profiles/r02_alu_peaks.txt is this output."""
+    import torch
+    import paper_1507_07733_b200.binding as B
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0); sampler.start()
+    pk = measure_alu_peaks(B)
+    clocks = sampler.stop()
+    hbm, src = load_peaks()
+    print(json.dumps({"alu_peaks": pk, "hbm_gbs": hbm, "hbm_source": src, "clocks": clocks,
+                      "derived_fp32_tflops_148sm_128lanes_1965mhz": FP32_PEAK_TFLOPS, "library": B.aera_version()}), flush=True)
+
+
 SCAN_FLOPS_PER_PAIR = 180000  # SURVEY 8(d-3): solve + two pruned inverse transforms + envelope per (direction, station)
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz (DESIGN.md 5.1)
 
@@ -193,6 +223,8 @@ def run_scan(args, wl):
     ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_SCAN, pat, B.AERA_F32, D, S, wl.n_samples, wl.fs_hz))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2, written between timed steps
     stream = torch.cuda.current_stream()
+    alu = measure_alu_peaks(B)["f32x2"]      # the "alu" roofline's denominator, measured on this device in this run
+    torch.cuda.synchronize()
 
     def step():
         B.aera_scan_directions(pat, d_tr, d_dirs, wl.fs_hz, peak_amp=amp, peak_idx=idx, workspace=ws, stream=stream)
@@ -238,10 +270,12 @@ def run_scan(args, wl):
         "config": {"workload": f"BASELINE configs[2] direction scan: 1 event x {S} stations x {D} directions", "n_dirs": D, "n_stations": S,
                    "n_samples": wl.n_samples, "l2_policy": "256 MB buffer written between timed steps (L2 flush)",
                    "kernel_variant": "auto" if args.variant == 0 else "generic"},
-        "roofline": {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP32_PEAK_TFLOPS, "traffic": None,
+        "roofline": {"bound": "alu", "achieved": ach, "peak": alu["tflops"], "unit": "TFLOP/s", "frac": ach / alu["tflops"], "traffic": None,
                      "kernel": "scan inverse (solve + 2 pruned iFFT + envelope argmax per pair)", "kernel_ms": k_avg,
                      "kernel_share_of_step": k_avg / ms_step, "scan_fwd_kernel_ms": f_ms / max(f_n, 1), "minv_kernel_ms": m_ms / max(m_n, 1),
-                     "algorithmic_flops_per_pair": SCAN_FLOPS_PER_PAIR, "peak_source": "derived: 148 SMs x 128 lanes x 2 x 1.965 GHz"},
+                     "algorithmic_flops_per_pair": SCAN_FLOPS_PER_PAIR,
+                     "peak_source": f"measured in this run: aera_measure_alu_peak(fma.rn.f32x2) = {alu['lane_fma_per_clk_per_sm']:.1f} lane-FMA/clk/SM x {alu['sm_count']} SMs x {alu['sm_clock_mhz']:.0f} MHz x 2",
+                     "derived_peak_tflops": FP32_PEAK_TFLOPS},
         "cpu_baseline": None,
         "e2e": {"value": pairs / t_e2e, "unit": "pairs/s", "h2d_bytes_per_step": int(tr_h.numel() * 4 + dirs_h.numel() * 8),
                 "d2h_bytes_per_step": int(pairs * 8), "ms_per_step": t_e2e * 1e3, "steps": n_e2e},
@@ -395,6 +429,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 auto, 1 generic)")
     ap.add_argument("--loop", type=int, default=0, help="config 1 only: time the device-resident reconstruction loop with this many iterations")
     ap.add_argument("--fold", action="store_true", help="time the on-device forward model (aera_fold_batch) on the config's shapes")
+    ap.add_argument("--peaks", action="store_true", help="measure and print the device's ALU issue peaks (packed fp32, fp32, fp64) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -403,6 +438,10 @@ def main():
 
     if args.impl == "reference":
         run_reference(args, wl)
+        return
+    if args.peaks:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_peaks(args)
         return
 
     if args.config == 2:

@@ -230,6 +230,22 @@ unsigned long long aera_launch_count(void);
 int aera_profile_enable(int on);
 aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches);
 
+/* Measured ALU throughput of the current device: the denominator of the "alu" roofline that bench.py reports for
+ * the FP32-pipe-bound direction scan (BASELINE north_star: "FP32/FP64 pipe utilisation for the scan mode"), in
+ * place of a number derived from unit counts and clocks. A register-only chain of independent fused multiply-adds
+ * on every SM (warps_per_sm warps each, 1..32) is timed with CUDA events (best of 3).
+ *   kind 0: packed fp32 (fma.rn.f32x2, the warp kernels' instruction), 1: scalar fp32, 2: fp64
+ *   lane_fma_per_s  out: fused multiply-adds per second over the whole device (x 2 = FLOP/s)
+ *   sm_count, sm_clock_khz  out: cudaDevAttrMultiProcessorCount, cudaDevAttrClockRate (may be NULL)
+ * SYNCHRONOUS (default stream); allocates and frees a small device buffer. Errors: INVALID_ARG, ALLOC/CUDA. */
+aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count, int *sm_clock_khz);
+
+/* Which kernel family the most recent aera_unfold_batch / aera_fold_batch / aera_scan_directions /
+ * aera_reconstruct_batch call of this thread dispatched to: a static string such as "unfold_w32<10,28>",
+ * "unfold_t4k_f64", "unfold_long_f32", "scan_w32", "generic" ("" before the first call). Lets a caller see that a
+ * size or band fell to the slower generic radix-2 kernels. */
+const char *aera_last_kernel(void);
+
 /* Message for the most recent non-OK status on this thread ("" if none). Static storage. */
 const char *aera_last_error(void);
 

@@ -21,7 +21,7 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
-           "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read")
+           "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel")
 
 
 class AeraError(RuntimeError):
@@ -82,6 +82,9 @@ def _load():
     lib.aera_profile_read.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
     lib.aera_profile_read.restype = C.c_int
     lib.aera_last_error.restype = C.c_char_p
+    lib.aera_last_kernel.restype = C.c_char_p
+    lib.aera_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), ip, ip]
+    lib.aera_measure_alu_peak.restype = C.c_int
     lib.aera_version.restype = C.c_char_p
     return lib, path
 
@@ -148,6 +151,21 @@ def aera_launch_count() -> int:
 
 def aera_set_kernel_variant(variant: int) -> int:
     return int(_lib.aera_set_kernel_variant(int(variant)))
+
+
+def aera_last_kernel() -> str:
+    """Kernel family the most recent unfold / fold / scan / reconstruct call of this thread dispatched to."""
+    return _lib.aera_last_kernel().decode()
+
+
+ALU_KINDS = {"f32x2": 0, "f32": 1, "f64": 2}
+
+
+def aera_measure_alu_peak(kind: int, warps_per_sm: int = 16):
+    """-> dict(lane_fma_per_s, sm_count, sm_clock_khz): measured FMA issue peak of the current device."""
+    v, n, khz = C.c_double(), C.c_int(), C.c_int()
+    _check(_lib.aera_measure_alu_peak(int(kind), int(warps_per_sm), C.byref(v), C.byref(n), C.byref(khz)))
+    return dict(lane_fma_per_s=v.value, sm_count=n.value, sm_clock_khz=khz.value)
 
 
 KERNEL_IDS = {"repack": 0, "minv": 1, "unfold": 2, "scan_fwd": 3, "scan_inv": 4, "timing": 5, "planefit": 6}

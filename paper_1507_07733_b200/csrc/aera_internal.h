@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of libaera_unfold.so.
 // Nothing here is part of the C ABI (include/aera_unfold.h) and nothing here is shared with oracle/.
 #pragma once
+#include <atomic>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
@@ -42,6 +43,25 @@ struct ProfScope {
     ProfScope(int k, cudaStream_t st) : kid(k), s(st) { prof_begin(kid, s); }
     ~ProfScope() { prof_end(kid, s); }
 };
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize raised once per kernel (and again only if a call needs more), not
+// on every launch: `cur` is a static of the call site, one per kernel instantiation.
+#define AERA_ENSURE_DYN_SMEM(kern, bytes)                                                                   \
+    do {                                                                                                    \
+        static std::atomic<size_t> aera_cur_smem{0};                                                        \
+        if ((size_t)(bytes) > aera_cur_smem.load(std::memory_order_acquire)) {                              \
+            cudaError_t aera_e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes)); \
+            if (aera_e != cudaSuccess) return aera_e;                                                       \
+            aera_cur_smem.store((size_t)(bytes), std::memory_order_release);                                \
+        }                                                                                                   \
+    } while (0)
+
+// ---- peaks.cu: measured ALU issue peaks (aera_measure_alu_peak)
+cudaError_t measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count, int *sm_clock_khz);
+// number of SMs of the current device (cached; api.cu)
+int sm_count();
+// records the kernel family a call dispatched to (aera_last_kernel)
+void note_kernel(const char *name);
 
 // ---- pattern.cu
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);

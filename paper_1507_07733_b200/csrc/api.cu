@@ -21,6 +21,22 @@ void count_launches(unsigned n) { g_launches.fetch_add(n, std::memory_order_rela
 int kernel_variant() { return g_variant.load(std::memory_order_relaxed); }
 
 static thread_local char g_err[512] = "";
+static thread_local const char *g_last_kernel = "";
+void note_kernel(const char *name) { g_last_kernel = name; }
+
+int sm_count()
+{
+    static std::atomic<int> cached{0};
+    int n = cached.load(std::memory_order_relaxed);
+    if (n > 0) return n;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        n = 148; // B200
+    }
+    cached.store(n, std::memory_order_relaxed);
+    return n;
+}
 
 // ---- per-kernel event timing -------------------------------------------------------------
 struct ProfRec { int kid; cudaEvent_t e0, e1; };
@@ -312,6 +328,20 @@ aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches)
 }
 
 const char *aera_last_error(void) { return g_err; }
+const char *aera_last_kernel(void) { return g_last_kernel; }
+
+aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count_out, int *sm_clock_khz)
+{
+    if (kind < 0 || kind > 2) return fail(AERA_ERR_INVALID_ARG, "kind=%d is not 0 (packed fp32), 1 (fp32) or 2 (fp64)", kind);
+    if (warps_per_sm < 1 || warps_per_sm > 32) return fail(AERA_ERR_INVALID_ARG, "warps_per_sm=%d must be in 1..32", warps_per_sm);
+    if (!lane_fma_per_s) return fail(AERA_ERR_INVALID_ARG, "lane_fma_per_s is NULL");
+    int sms = 0, khz = 0;
+    cudaError_t e = measure_alu_peak(kind, warps_per_sm, lane_fma_per_s, &sms, &khz);
+    if (e != cudaSuccess) return cuda_fail(e, "ALU peak measurement");
+    if (sm_count_out) *sm_count_out = sms;
+    if (sm_clock_khz) *sm_clock_khz = khz;
+    return AERA_OK;
+}
 const char *aera_version(void) { return "aera_unfold 0.1 (sm_100a)"; }
 unsigned long long aera_launch_count(void) { return g_launches.load(); }
 int aera_set_kernel_variant(int variant) { return g_variant.exchange(variant); }
@@ -455,6 +485,7 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
                                 warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS)),
                                 ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s, forward);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
+    note_kernel(warp_path ? "unfold_w32" : (team_path ? "unfold_t4k_f64" : (long_path ? "unfold_long_f32" : "generic")));
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s,
                               spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode);
@@ -515,6 +546,7 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
     cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_dirs, ws + w.off_minv,
                                 warp_path ? MINV_PACKED : MINV_ROWS, (warp_path ? 1.0 : 2.0) / (double)n_samples, s);
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
+    note_kernel(warp_path ? "scan_w32" : "generic");
     if (warp_path)
         e = launch_scan_w32(pl->dev, n_stations, traces, n_dirs, ws + w.off_minv, peak_amp, peak_idx, ws + w.off_spectra, s);
     else

@@ -114,7 +114,7 @@ cudaError_t launch_timing(int dtype, const void *traces, long n_units, int N, in
     if (n_units <= 0) return cudaSuccess;
     ProfScope prof(KID_TIMING, s);
     long grid = (n_units + 7) / 8;
-    if (grid > 148L * 8) grid = 148L * 8;
+    if (grid > (long)sm_count() * 8) grid = (long)sm_count() * 8;
     if (dtype == AERA_F32) timing_kernel<float><<<(unsigned)grid, 256, 0, s>>>((const float *)traces, n_units, N, idx0, (float *)w0);
     else timing_kernel<double><<<(unsigned)grid, 256, 0, s>>>((const double *)traces, n_units, N, idx0, (double *)w0);
     count_launches(1);

@@ -35,7 +35,7 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
     ProfScope prof(KID_REPACK, s);
     size_t total = (size_t)n_z * n_a * n_f * 4;
     int blocks = (int)((total + 255) / 256);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     if (dtype == AERA_F32)
         repack_kernel<float><<<blocks, 256, 0, s>>>((const cx<float> *)src, (cx<float> *)dst, n_z, n_a, n_f);
     else
@@ -190,13 +190,11 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
     size_t smem = minv_smem_bytes(dtype, g.n_f);
     cudaError_t e;
     if (dtype == AERA_F32) {
-        e = cudaFuncSetAttribute(minv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        AERA_ENSURE_DYN_SMEM(minv_kernel<float>, smem);
         minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
                                                              p.K, scale, layout, p.k_lo, forward, (cx<float> *)minv);
     } else {
-        e = cudaFuncSetAttribute(minv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        AERA_ENSURE_DYN_SMEM(minv_kernel<double>, smem);
         minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
                                                               p.K, scale, layout, p.k_lo, forward, (cx<double> *)minv);
     }

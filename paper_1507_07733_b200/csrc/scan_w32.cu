@@ -311,8 +311,7 @@ cudaError_t launch_scan_w32(const PlanDev &p, int n_stations, const void *traces
         ProfScope prof(KID_SCAN_FWD, s);
         const size_t smem = (size_t)kTabBytes + 4 * (size_t)G::kWarpBytes;
         auto kern = scan_fwd_w32_kernel<10, 28>;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        AERA_ENSURE_DYN_SMEM(kern, smem);
         kern<<<(unsigned)((n_stations + 3) / 4), 128, smem, s>>>(q);
     }
     {
@@ -320,10 +319,9 @@ cudaError_t launch_scan_w32(const PlanDev &p, int n_stations, const void *traces
         const size_t slot = ((size_t)kScanDirs * p.K * 32 + 127) & ~(size_t)127;
         const size_t smem = (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)ScanGeom<10, 28>::kWarps * kXBytes;
         auto kern = scan_inv_w32_kernel<10, 28>;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        AERA_ENSURE_DYN_SMEM(kern, smem);
         const long n_tiles = (long)((n_stations + kScanStations - 1) / kScanStations) * ((n_dirs + kScanDirs - 1) / kScanDirs);
-        const long grid = n_tiles < 148 ? n_tiles : 148;
+        const long grid = n_tiles < sm_count() ? n_tiles : sm_count();
         kern<<<(unsigned)grid, ScanGeom<10, 28>::kWarps * 32, smem, s>>>(q);
     }
     count_launches(2);

@@ -226,7 +226,7 @@ scan_inverse_generic_kernel(PlanDev p, int n_stations, long n_pairs, const cx<T>
 
 size_t elem_bytes(int dtype) { return dtype == AERA_F32 ? sizeof(cx<float>) : sizeof(cx<double>); }
 bool fits_smem(int dtype, int N) { return (size_t)3 * N * elem_bytes(dtype) <= kSmemBudget; }
-long generic_grid(long n_units) { return n_units < 148L * 4 ? n_units : 148L * 4; }
+long generic_grid(long n_units) { return n_units < (long)sm_count() * 4 ? n_units : (long)sm_count() * 4; }
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes)

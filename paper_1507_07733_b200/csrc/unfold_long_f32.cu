@@ -40,7 +40,7 @@ constexpr int kLN = 65536;
 constexpr int kLWarps = 4;                 // warps per CTA
 constexpr int kLCtasPerSm = 3;             // 12 warps per SM, from three different stations (phases decoupled)
 constexpr int kLCluster = 8;               // CTAs per station (thread-block cluster): 32 warps, every phase (32 tasks) is ONE round
-constexpr int kLMaxClusters = 148 * kLCtasPerSm / kLCluster;   // 55 stations in flight
+inline int long_max_clusters() { return sm_count() * kLCtasPerSm / kLCluster; }   // 55 stations in flight on 148 SMs
 constexpr int kLTeam = kLWarps * kLCluster;
 constexpr size_t kYBytes = (size_t)32 * 1024 * 16;            // Y[q][mm] two 8-byte planes; reused as U[2][16][1024]
 // band geometry of the one instantiation (configs[4]: k = 1311 .. 13107)
@@ -447,7 +447,7 @@ static size_t long_stride(const PlanDev &p)
     const size_t C = (size_t)((p.k_hi >> 5) - (p.k_lo >> 5) + 1);
     return (kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | per-CTA peaks
 }
-size_t long_f32_scratch_bytes(const PlanDev &p) { return kLMaxClusters * long_stride(p); }
+size_t long_f32_scratch_bytes(const PlanDev &p) { return long_max_clusters() * long_stride(p); }
 
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                    void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
@@ -464,19 +464,18 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
     const size_t smem = 8192 + 4096 + 128 + (size_t)kLWarps * kXBytes;
     cudaError_t e;
     auto launch = [&](auto kern) -> cudaError_t {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        AERA_ENSURE_DYN_SMEM(kern, smem);
         // persistent clusters: as many as can be co-resident (a cluster of 8 must fit one GPC), at most one per station
         static int max_clusters = 0;                       // same for both instantiations to within rounding; cached
         if (max_clusters == 0) {
             cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3(kLCluster * kLMaxClusters); cfg.blockDim = dim3(kLWarps * 32); cfg.dynamicSmemBytes = smem;
+            cfg.gridDim = dim3(kLCluster * long_max_clusters()); cfg.blockDim = dim3(kLWarps * 32); cfg.dynamicSmemBytes = smem;
             cudaLaunchAttribute at[1];
             at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = kLCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
             cfg.attrs = at; cfg.numAttrs = 1;
             int n = 0;
-            if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) { (void)cudaGetLastError(); n = kLMaxClusters; }
-            max_clusters = n < kLMaxClusters ? n : kLMaxClusters;
+            if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) { (void)cudaGetLastError(); n = long_max_clusters(); }
+            max_clusters = n < long_max_clusters() ? n : long_max_clusters();
             if (getenv("AERA_DEBUG")) fprintf(stderr, "[aera] long-trace kernel: %d co-resident clusters of %d CTAs (occupancy query %d)\n", max_clusters, kLCluster, n);
         }
         const long clusters = n_units < max_clusters ? n_units : max_clusters;

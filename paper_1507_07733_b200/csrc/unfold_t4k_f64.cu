@@ -435,10 +435,9 @@ cudaError_t launch_t4k(const T4kParams &q, cudaStream_t s)
 {
     const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * kTeamBytes;
     auto kern = unfold_t4k_f64_kernel<RLO, RHI, HAS_EF>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + kTeams - 1) / kTeams;
-    if (grid > 148) grid = 148;
+    if (grid > sm_count()) grid = sm_count();
     kern<<<(unsigned)grid, kTeams * kTeamThreads, smem, s>>>(q);
     return cudaGetLastError();
 }

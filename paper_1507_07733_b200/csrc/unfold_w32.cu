@@ -330,10 +330,9 @@ cudaError_t launch_inst(const W32Params &q, cudaStream_t s)
     using G = W32Geom<K2LO, K2HI>;
     const size_t smem = w32_smem_bytes<K2LO, K2HI, MINV_SMEM>(q.K);
     auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, SPEC>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + G::kWarps - 1) / G::kWarps;
-    if (grid > 148) grid = 148;
+    if (grid > sm_count()) grid = sm_count();
     kern<<<(unsigned)grid, G::kWarps * 32, smem, s>>>(q);
     return cudaGetLastError();
 }
