@@ -38,8 +38,19 @@
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
 #include "w32_common.cuh"
 
+#ifndef AERA_PREFETCH_DIST
+#define AERA_PREFETCH_DIST 1
+#endif
+#ifndef AERA_FFT_LOOP_FORM
+#define AERA_FFT_LOOP_FORM 0
+#endif
+#ifndef AERA_SOLVE_UNROLL
+#define AERA_SOLVE_UNROLL 1
+#endif
 namespace aera {
 namespace {
+
+constexpr int kSolveUnroll = AERA_SOLVE_UNROLL;   // band rows of separate_solve in flight together
 
 struct W32Params {
     const float *traces;
@@ -70,33 +81,36 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
     int own = (G::kLo - G::kPubLo) * 32 + lane;
     int par = (31 - G::kLo + (lane == 0 ? 1 : 0) - G::kPubLo) * 32 + ((32 - lane) & 31);
     int k = lane + 32 * G::kLo;
-#pragma unroll 1
+#pragma unroll (kSolveUnroll)
     for (int r = 0; r < G::kBandRows; ++r, own += 32, par -= 32, k += 32) {
-        R er = L::zero(), ei = L::zero();
-        float4 vsp = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (k >= k_lo && k <= k_hi) {
-            const R ar = QA[own], ai = QB[own], pr = QA[par], pi = QB[par];
-            // F'_0 = G + conj(Gm) = 2 FFT(v0 polyphase r), F'_1 = -i (G - conj(Gm)) = 2 FFT(v1 polyphase r)
-            const R f0r = L::add(ar, pr), f0i = L::sub(ai, pi);
-            const R f1r = L::add(ai, pi), f1i = L::sub(pr, ar);
-            float f0r0, f0r1, f0i0, f0i1, f1r0, f1r1, f1i0, f1i1;
-            L::unpack(f0r, f0r0, f0r1); L::unpack(f0i, f0i0, f0i1);
-            L::unpack(f1r, f1r0, f1r1); L::unpack(f1i, f1i0, f1i1);
-            const float2 w = TS[k]; // W_2048^k = (wr, wi)
-            float v0r = fmaf(w.x, f0r1, f0r0); v0r = fmaf(-w.y, f0i1, v0r);
-            float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
-            float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
-            float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
-            if (SPEC == 1) vsp = make_float4(v0r, v0i, v1r, v1i);
-            const float4 m0 = MINV_SMEM ? MA[k - k_lo] : ld_nc_f4(MA + (k - k_lo));
-            const float4 m1 = MINV_SMEM ? MB[k - k_lo] : ld_nc_f4(MB + (k - k_lo));
-            const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
-            er = L::mul(Ma, L::bc(v0r)); er = L::fma(Mb, L::bc(-v0i), er);
-            er = L::fma(Mc, L::bc(v1r), er); er = L::fma(Md, L::bc(-v1i), er);
-            ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
-            ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
-        }
-        if (SPEC == 1) sp[r * 32] = vsp;
+        // branch-free: rows at the band edges read a clamped Minv entry and select zero afterwards, so the
+        // loads of neighbouring rows are independent and the unrolled iterations overlap their latencies
+        const bool inband = k >= k_lo && k <= k_hi;
+        int j = k - k_lo;
+        j = j < 0 ? 0 : (j > k_hi - k_lo ? k_hi - k_lo : j);
+        // (lane 0 of row 0 would look for its mirror in row 32: k = 0 is never in band, keep the read inside the buffer)
+        const int pc = (G::kLo == 0 && par > G::kPubRows * 32 - 1) ? G::kPubRows * 32 - 1 : par;
+        const R ar = QA[own], ai = QB[own], pr = QA[pc], pi = QB[pc];
+        const float2 w = TS[k]; // W_2048^k = (wr, wi)
+        const float4 m0 = MINV_SMEM ? MA[j] : ld_nc_f4(MA + j);
+        const float4 m1 = MINV_SMEM ? MB[j] : ld_nc_f4(MB + j);
+        // F'_0 = G + conj(Gm) = 2 FFT(v0 polyphase r), F'_1 = -i (G - conj(Gm)) = 2 FFT(v1 polyphase r)
+        const R f0r = L::add(ar, pr), f0i = L::sub(ai, pi);
+        const R f1r = L::add(ai, pi), f1i = L::sub(pr, ar);
+        float f0r0, f0r1, f0i0, f0i1, f1r0, f1r1, f1i0, f1i1;
+        L::unpack(f0r, f0r0, f0r1); L::unpack(f0i, f0i0, f0i1);
+        L::unpack(f1r, f1r0, f1r1); L::unpack(f1i, f1i0, f1i1);
+        float v0r = fmaf(w.x, f0r1, f0r0); v0r = fmaf(-w.y, f0i1, v0r);
+        float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
+        float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
+        float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
+        if (!inband) { v0r = 0.f; v0i = 0.f; v1r = 0.f; v1i = 0.f; }
+        const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
+        R er = L::mul(Ma, L::bc(v0r)); er = L::fma(Mb, L::bc(-v0i), er);
+        er = L::fma(Mc, L::bc(v1r), er); er = L::fma(Md, L::bc(-v1i), er);
+        R ei = L::mul(Ma, L::bc(v0i)); ei = L::fma(Mb, L::bc(v0r), ei);
+        ei = L::fma(Mc, L::bc(v1i), ei); ei = L::fma(Md, L::bc(v1r), ei);
+        if (SPEC == 1) sp[r * 32] = make_float4(v0r, v0i, v1r, v1i);
         tmem_st64(tstash + 4 * r, er.v);
         tmem_st64(tstash + 4 * r + 2, ei.v);
     }
@@ -203,8 +217,8 @@ unfold_w32_kernel(W32Params p)
             const float *v = p.traces + (size_t)u * 4 * kM;
             float *ef = HAS_EF ? p.efield + (size_t)u * 4 * kM : nullptr;
             float4 *sp = SPEC != 0 ? p.spectra + (size_t)u * G::kBandRows * 32 + lane : nullptr;
-            if (lane == 0 && u + kWarps < u1) {
-                if (SPEC != 2) prefetch_l2_bulk(v + (size_t)kWarps * 4 * kM, 4 * kM * sizeof(float));
+            if (AERA_PREFETCH_DIST > 0 && lane == 0 && u + AERA_PREFETCH_DIST * kWarps < u1) {
+                if (SPEC != 2) prefetch_l2_bulk(v + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(float));
                 else prefetch_l2_bulk(p.spectra + (size_t)(u + kWarps) * G::kBandRows * 32, G::kBandRows * 32 * sizeof(float4));
             }
 
@@ -236,8 +250,25 @@ unfold_w32_kernel(W32Params p)
             int t = SPEC == 2 ? 1 : 0;
 #pragma unroll 1
             for (;;) {
+#if AERA_FFT_LOOP_FORM == 1
+                // two passes of 32-point FFTs through ONE copy of their code: a bottom-tested loop whose body is the
+                // FFT followed by the conditional inter-pass work (a loop with the exit test in the middle is rotated
+                // by the compiler, which duplicates the 388-instruction FFT); the counter is opaque to the optimiser
+                int pass = 0;
+#pragma unroll 1
+                do {
+                    fft32<L>(A, B);
+                    asm volatile("" : "+r"(pass));
+                    if (pass == 0) {
+                        pass_twiddle(A, B, T, lane);
+                        transpose_plane(A, X, lane);
+                        transpose_plane(B, X, lane);
+                    }
+                    ++pass;
+                } while (pass < 2);
+#else
                 int second = 0;
-                asm volatile("" : "+r"(second)); // opaque trip count: keeps ONE copy of the 32-point FFT
+                asm volatile("" : "+r"(second));
 #pragma unroll 1
                 for (;;) {
                     fft32<L>(A, B);
@@ -248,6 +279,7 @@ unfold_w32_kernel(W32Params p)
                     second = 1;
                     asm volatile("" : "+r"(second));
                 }
+#endif
                 if (t == 2) break;
                 if (SPEC != 2 && t == 0) {
                     // ---- a2 done: publish the band rows and the rows that are somebody's bin 1024-k
