@@ -38,6 +38,9 @@
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
 #include "w32_common.cuh"
 
+#ifndef AERA_W32_ABLATE
+#define AERA_W32_ABLATE 0   // timing experiments only (wrong results), bit mask: 1 no fft32, 2 no transposes, 4 no global loads/stores, 8 no pass twiddles, 16 no separation+solve, 32 no envelope/argmax
+#endif
 #ifndef AERA_PREFETCH_DIST
 #define AERA_PREFETCH_DIST 1
 #endif
@@ -227,6 +230,7 @@ unfold_w32_kernel(W32Params p)
                 // ---- a1: the station's two traces, read once, straight into FFT input order
                 static_for<0, 32>([&](auto jc) {
                     constexpr int j = decltype(jc)::value;
+                    if (AERA_W32_ABLATE & 4) { A[brev5(j)] = L::pack(lane * 0.5f, j); B[brev5(j)] = L::pack(j, lane); return; }
                     A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
                     B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
                 });
@@ -271,11 +275,13 @@ unfold_w32_kernel(W32Params p)
                 asm volatile("" : "+r"(second));
 #pragma unroll 1
                 for (;;) {
-                    fft32<L>(A, B);
+                    if (!(AERA_W32_ABLATE & 1)) fft32<L>(A, B);
                     if (second) break;
-                    pass_twiddle(A, B, T, lane);
+                    if (!(AERA_W32_ABLATE & 8)) pass_twiddle(A, B, T, lane);
+                    if (!(AERA_W32_ABLATE & 2)) {
                     transpose_plane(A, X, lane);
                     transpose_plane(B, X, lane);
+                    }
                     second = 1;
                     asm volatile("" : "+r"(second));
                 }
@@ -293,7 +299,7 @@ unfold_w32_kernel(W32Params p)
                     // ---- separate channels, fold the two polyphase halves, a4: E = Minv V, one band
                     // row per iteration (a rolled loop: 40 instructions instead of 19 x 45), E goes to
                     // this lane's tensor-memory columns and is read back twice (s = 0, 1)
-                    separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MA, MB, p.k_lo, p.k_hi, lane, tstash, sp);
+                    if (!(AERA_W32_ABLATE & 16)) separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MA, MB, p.k_lo, p.k_hi, lane, tstash, sp);
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
                     // ---- a5: even samples  z[2m] = IFFT_1024(E): inverse roles, A = Im, B = Re

@@ -73,8 +73,12 @@ __device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const floa
     fft32<L>(A, B);
 }
 
+#ifndef AERA_W32_ABLATE
+#define AERA_W32_ABLATE 0   // timing experiments only, see unfold_w32.cu
+#endif
 __device__ __forceinline__ void st_global_b64(void *p, R v)
 {
+    if ((AERA_W32_ABLATE & 4) && v.v != 0x123456789abcdefull) return;
     asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
 }
 
