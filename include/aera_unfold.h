@@ -166,6 +166,60 @@ aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_ev
                               void *traces, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * Several pattern tables, one antenna type per station (section 3: "The patterns for all antennas used in
+ * AERA can be stored simultaneously on the device"; L43: "For each antenna, the VEL is known for discrete frequencies and
+ * zenith and azimuth angles"). Exactly aera_unfold_batch, except that station s of every event is unfolded with the table
+ * patterns[pattern_id[s]]; the per-direction matrices are then built once per (event, table).
+ *   patterns    HOST array of n_patterns handles (1..64), all of the call's dtype and with the same frequency axis
+ *               (n_freq, freq0_hz, dfreq_hz: the in-band bins must agree); zenith / azimuth grids may differ
+ *   pattern_id  DEVICE [n_stations] int32, values in 0 .. n_patterns-1 (not checked on the device)
+ *   workspace   >= aera_workspace_bytes_ex(AERA_OP_UNFOLD, patterns[0], dtype, n_events, n_stations, n_samples, fs_hz,
+ *               n_patterns, 1)
+ * A band filter set on patterns[0] applies to all tables. Errors as aera_unfold_batch.
+ */
+aera_status_t aera_unfold_batch_multi(const aera_pattern_t *const *patterns, int n_patterns, const int32_t *pattern_id,
+                                      int dtype, int n_events, int n_stations, int n_samples, double fs_hz,
+                                      const void *traces, const double *dirs, void *efield, void *peak_amp, int32_t *peak_idx,
+                                      void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * int16 ADC-count input (section 2: "the voltage traces of the two channels at each station are read out";
+ * the station electronics deliver ADC counts, the paper does not give the conversion). The traces are read as int16, which
+ * halves the bytes read per station (24 584 algorithmic bytes per unit at n_samples = 2048 instead of 32 776):
+ *     v_c[n] = counts_to_volts[c] * traces[..][c][n]       then exactly aera_unfold_batch in fp32
+ * (the two factors are folded into the per-direction matrices: the unfolding is linear in the traces).
+ *   traces           DEVICE [n_events][n_stations][2][n_samples] int16, 16-byte aligned
+ *   counts_to_volts  HOST [2] double, one factor per channel
+ *   efield / peak_amp / peak_idx  as aera_unfold_batch with dtype AERA_F32 (efield cannot alias traces)
+ *   pattern          an AERA_F32 pattern; workspace >= aera_workspace_bytes(AERA_OP_UNFOLD, pattern, AERA_F32, ...)
+ */
+aera_status_t aera_unfold_batch_i16(const aera_pattern_t *pattern, int n_events, int n_stations, int n_samples, double fs_hz,
+                                    const int16_t *traces, const double *counts_to_volts, const double *dirs,
+                                    float *efield, float *peak_amp, int32_t *peak_idx,
+                                    void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * Spectral up-sampling by zero-padding (section 2: "after noise filtering and signal enhancing"; the paper
+ * does not specify the enhancement, reading R23): the unfolded band spectrum is unchanged and the analytic signal
+ * is evaluated on a grid `upsample` times finer,
+ *     z_p[n] = (2/N) sum_{k in band} E_p[k] exp(+2 pi i n k / (upsample N)),   n = 0 .. upsample N - 1,
+ * so that z[upsample n] is the sample n of aera_unfold_batch and the envelope maximum is found with sub-sample timing.
+ *   upsample  power of two >= 1 with upsample * n_samples <= 65536
+ *   efield    DEVICE [n_events][n_stations][2][upsample * n_samples] (may be NULL; cannot alias traces unless upsample == 1)
+ *   peak_idx  index on the FINE grid (0 .. upsample * n_samples - 1), peak_amp the envelope maximum there
+ *   workspace >= aera_workspace_bytes_ex(AERA_OP_UNFOLD, pattern, dtype, n_events, n_stations, n_samples, fs_hz, 1, upsample)
+ * upsample > 1 runs on the generic kernels (aera_last_kernel() says so).
+ */
+aera_status_t aera_unfold_batch_upsampled(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations, int n_samples,
+                                          double fs_hz, int upsample, const void *traces, const double *dirs,
+                                          void *efield, void *peak_amp, int32_t *peak_idx,
+                                          void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* aera_workspace_bytes for the calls above: n_patterns tables (1 for a single one), spectral up-sampling factor (1 = none). */
+size_t aera_workspace_bytes_ex(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,
+                               int n_stations, int n_samples, double fs_hz, int n_patterns, int upsample);
+
+/*
  * Device-resident reconstruction loop (section 2, L29 and Fig. 1: "First, as an initial estimate of the
  * event timing in each station, the maxima of the voltage traces is used. Second, from the timing information of
  * the individual stations, the direction of the shower is obtained by triangulation. Third, the antenna pattern

@@ -21,7 +21,8 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
-           "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel")
+           "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel", "aera_unfold_batch_multi", "aera_unfold_batch_i16",
+           "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex")
 
 
 class AeraError(RuntimeError):
@@ -82,6 +83,14 @@ def _load():
     lib.aera_profile_read.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
     lib.aera_profile_read.restype = C.c_int
     lib.aera_last_error.restype = C.c_char_p
+    lib.aera_unfold_batch_multi.argtypes = [C.POINTER(vp), C.c_int, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.aera_unfold_batch_multi.restype = C.c_int
+    lib.aera_unfold_batch_i16.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, vp, C.POINTER(C.c_double), dp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.aera_unfold_batch_i16.restype = C.c_int
+    lib.aera_unfold_batch_upsampled.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, vp, dp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.aera_unfold_batch_upsampled.restype = C.c_int
+    lib.aera_workspace_bytes_ex.argtypes = [C.c_int, vp, C.c_int, C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int]
+    lib.aera_workspace_bytes_ex.restype = C.c_size_t
     lib.aera_last_kernel.restype = C.c_char_p
     lib.aera_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), ip, ip]
     lib.aera_measure_alu_peak.restype = C.c_int
@@ -218,6 +227,14 @@ def aera_workspace_bytes(op: int, p: Pattern, dtype: int, n_events_or_dirs: int,
     return n
 
 
+def aera_workspace_bytes_ex(op: int, p: Pattern, dtype: int, n_events_or_dirs: int, n_stations: int, n_samples: int, fs_hz: float,
+                            n_patterns: int = 1, upsample: int = 1) -> int:
+    n = int(_lib.aera_workspace_bytes_ex(op, p.handle, dtype, n_events_or_dirs, n_stations, n_samples, fs_hz, n_patterns, upsample))
+    if n == 0:
+        raise AeraError(1, _lib.aera_last_error().decode())
+    return n
+
+
 def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:
     return torch.empty(nbytes, dtype=torch.uint8, device=device)
 
@@ -239,6 +256,63 @@ def aera_unfold_batch(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_h
         workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, traces.device)
     _check(_lib.aera_unfold_batch(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp),
                                   _ptr(peak_idx), _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return efield, peak_amp, peak_idx
+
+
+def _outputs(traces, E, S, n_out, efield, peak_amp, peak_idx, want_efield, out_dtype):
+    if efield is None and want_efield:
+        efield = torch.empty((E, S, 2, n_out), dtype=out_dtype, device=traces.device)
+    if peak_amp is None:
+        peak_amp = torch.empty((E, S), dtype=out_dtype, device=traces.device)
+    if peak_idx is None:
+        peak_idx = torch.empty((E, S), dtype=torch.int32, device=traces.device)
+    return efield, peak_amp, peak_idx
+
+
+def aera_unfold_batch_multi(patterns, pattern_id: torch.Tensor, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float,
+                            efield=None, peak_amp=None, peak_idx=None, workspace=None, stream=None, want_efield=True):
+    """patterns: list of Pattern; pattern_id [S] CUDA int32 (antenna type per station); otherwise as aera_unfold_batch."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    assert pattern_id.is_cuda and pattern_id.dtype == torch.int32 and tuple(pattern_id.shape) == (S,) and pattern_id.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    efield, peak_amp, peak_idx = _outputs(traces, E, S, N, efield, peak_amp, peak_idx, want_efield, traces.dtype)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes_ex(AERA_OP_UNFOLD, patterns[0], dt, E, S, N, fs_hz, len(patterns), 1) if E > 0 else 256, traces.device)
+    handles = (C.c_void_p * len(patterns))(*[p.handle for p in patterns])
+    _check(_lib.aera_unfold_batch_multi(handles, len(patterns), _ptr(pattern_id), dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield),
+                                        _ptr(peak_amp), _ptr(peak_idx), _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return efield, peak_amp, peak_idx
+
+
+def aera_unfold_batch_i16(p: Pattern, traces: torch.Tensor, counts_to_volts, dirs: torch.Tensor, fs_hz: float, efield=None,
+                          peak_amp=None, peak_idx=None, workspace=None, stream=None, want_efield=True):
+    """traces [E][S][2][N] CUDA int16 ADC counts, counts_to_volts (g0, g1). Returns fp32 (efield|None, peak_amp, peak_idx)."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous() and traces.dtype == torch.int16
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    efield, peak_amp, peak_idx = _outputs(traces, E, S, N, efield, peak_amp, peak_idx, want_efield, torch.float32)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, AERA_F32, E, S, N, fs_hz) if E > 0 else 256, traces.device)
+    g = (C.c_double * 2)(float(counts_to_volts[0]), float(counts_to_volts[1]))
+    _check(_lib.aera_unfold_batch_i16(p.handle, E, S, N, fs_hz, _ptr(traces), g, _ptr(dirs), _ptr(efield), _ptr(peak_amp), _ptr(peak_idx),
+                                      _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return efield, peak_amp, peak_idx
+
+
+def aera_unfold_batch_upsampled(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, upsample: int, efield=None,
+                                peak_amp=None, peak_idx=None, workspace=None, stream=None, want_efield=True):
+    """As aera_unfold_batch with the outputs on a grid `upsample` times finer: efield [E][S][2][upsample N]."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    dt = _dtype_code(traces.dtype)
+    efield, peak_amp, peak_idx = _outputs(traces, E, S, N * upsample, efield, peak_amp, peak_idx, want_efield, traces.dtype)
+    if workspace is None:
+        workspace = alloc_workspace(aera_workspace_bytes_ex(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz, 1, upsample) if E > 0 else 256, traces.device)
+    _check(_lib.aera_unfold_batch_upsampled(p.handle, dt, E, S, N, fs_hz, upsample, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp),
+                                            _ptr(peak_idx), _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
     return efield, peak_amp, peak_idx
 
 

@@ -29,6 +29,16 @@ struct PlanDev {
     const void *tw;         // [N/2] cx<T>: W_N^m = exp(-2 pi i m / N), m < N/2 (generic kernel)
     const void *tw1024;     // [1024] cx<T>: W_1024^m (warp kernels: 32x32 inter-pass twiddles)
     const void *twN;        // [N] cx<T>: W_N^m, m < N (real-FFT split / polyphase twiddles)
+    int U, logM;            // spectral up-sampling factor (1 = none) and log2(U N)
+    const void *twU;        // [U N / 2] cx<T>: W_{UN}^m (generic kernel's inverse transform on the fine grid; = tw when U = 1)
+};
+
+// Variations of the batch unfolding beyond one table / real-typed traces / the input sampling grid
+// (aera_unfold_batch_multi, aera_unfold_batch_i16, aera_unfold_batch_upsampled).
+struct UnfoldExt {
+    const int32_t *pattern_id = nullptr; // device [n_stations]: antenna type of each station (nullptr: one table)
+    size_t minv_pattern_stride = 0;      // complex elements between the Minv slabs of consecutive tables (= n_events * per-event size)
+    int input_i16 = 0;                   // traces are int16 ADC counts (the counts-to-volts factors are folded into Minv)
 };
 
 void count_launches(unsigned n);
@@ -79,14 +89,15 @@ enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3 };
 __host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
                         const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s,
-                        int forward = 0 /* 1: scale * H (forward model) instead of scale * H^-1 */);
+                        int forward = 0 /* 1: scale * H (forward model) instead of scale * H^-1 */,
+                        double chan_scale0 = 1.0, double chan_scale1 = 1.0 /* per-channel input scale folded into the columns */);
 size_t minv_smem_bytes(int dtype, int n_f);
 
 // ---- unfold_generic.cu
-size_t generic_scratch_bytes(int dtype, int N, long n_units);   // per-call global transform buffers (0 if smem-resident)
+size_t generic_scratch_bytes(int dtype, int N, long n_units, int upsample = 1);   // per-call global transform buffers (0 if smem-resident)
 cudaError_t launch_unfold_generic(int dtype, const PlanDev &p, long n_events, int n_stations,
                                   const void *traces, void *efield, void *amp, int32_t *idx,
-                                  const void *minv, void *scratch, cudaStream_t s);
+                                  const void *minv, void *scratch, cudaStream_t s, const UnfoldExt &x = UnfoldExt());
 size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations);
 cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, const void *traces,
                                 long n_dirs, const void *minv, void *amp, int32_t *idx,
@@ -98,18 +109,20 @@ bool w32_supported(int dtype, const PlanDev &p);
 // read, no forward transform); w32_spectra_bytes() = 0 when the band geometry has no such instantiation
 size_t w32_spectra_bytes(const PlanDev &p, long n_units);
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra = nullptr, int spec_mode = 0);
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra = nullptr, int spec_mode = 0,
+                              const UnfoldExt &x = UnfoldExt());
 
 // ---- unfold_t4k_f64.cu: team-per-station kernel for N = 4096 fp64, band rows 4..12 (configs[3])
 bool t4k_f64_supported(int dtype, const PlanDev &p);
 cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s);
+                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x = UnfoldExt());
 
 // ---- unfold_long_f32.cu: multi-pass kernel for N = 65536 fp32 through an L2-resident scratch (configs[4])
 bool long_f32_supported(int dtype, const PlanDev &p);
 size_t long_f32_scratch_bytes(const PlanDev &p);
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                                   void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s);
+                                   void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s,
+                                   const UnfoldExt &x = UnfoldExt());
 
 // ---- loop.cu: the two small steps that close the reconstruction loop on the device
 cudaError_t launch_timing(int dtype, const void *traces, long n_units, int N, int32_t *idx0, void *w0, cudaStream_t s);

@@ -110,7 +110,7 @@ struct aera_pattern {
     void *d_table = nullptr;
     size_t table_bytes = 0;
     std::mutex mu;
-    std::map<std::pair<int, double>, Plan *> plans;
+    std::map<std::pair<long long, double>, Plan *> plans;   // key: (n_samples | up-sampling factor << 32, fs)
     HostPipe pipe;
 };
 
@@ -175,10 +175,10 @@ void fill_twiddles(cx<T> *dst, int count, int N)
 }
 
 // Build (or fetch) the plan for (N, fs). May allocate and synchronise `s` on first use.
-aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan **out)
+aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan **out, int U = 1)
 {
     std::lock_guard<std::mutex> lk(pat->mu);
-    auto key = std::make_pair(N, fs);
+    auto key = std::make_pair((long long)N | ((long long)U << 32), fs);
     auto it = pat->plans.find(key);
     if (it != pat->plans.end()) { *out = it->second; return AERA_OK; }
 
@@ -189,13 +189,14 @@ aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan
     const int dtype = pat->desc.dtype;
     const size_t cb = cplx_bytes(dtype);
 
-    // blob layout: bin_if [K] | bin_tf [K] | tw [N/2] | tw1024 [1024] | twN [N]
+    // blob layout: bin_if [K] | bin_tf [K] | tw [N/2] | tw1024 [1024] | twN [N] | twU [U N / 2] (U > 1 only)
     size_t off_if = 0;
     size_t off_tf = align_up(off_if + sizeof(int) * K);
     size_t off_tw = align_up(off_tf + sizeof(double) * K);
     size_t off_t1k = align_up(off_tw + cb * (N / 2));
     size_t off_twN = align_up(off_t1k + cb * 1024);
-    size_t total = align_up(off_twN + cb * N);
+    size_t off_twU = align_up(off_twN + cb * N);
+    size_t total = U > 1 ? align_up(off_twU + cb * ((size_t)U * N / 2)) : off_twU;
     std::vector<unsigned char> h(total, 0);
     int *bin_if = reinterpret_cast<int *>(h.data() + off_if);
     double *bin_tf = reinterpret_cast<double *>(h.data() + off_tf);
@@ -212,10 +213,12 @@ aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan
         fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_tw), N / 2, N);
         fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_t1k), 1024, 1024);
         fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_twN), N, N);
+        if (U > 1) fill_twiddles(reinterpret_cast<cx<float> *>(h.data() + off_twU), U * N / 2, U * N);
     } else {
         fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_tw), N / 2, N);
         fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_t1k), 1024, 1024);
         fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_twN), N, N);
+        if (U > 1) fill_twiddles(reinterpret_cast<cx<double> *>(h.data() + off_twU), U * N / 2, U * N);
     }
     Plan *pl = new (std::nothrow) Plan();
     if (!pl) return fail(AERA_ERR_ALLOC, "host allocation of a plan failed");
@@ -233,6 +236,8 @@ aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan
     pl->dev.tw = b + off_tw;
     pl->dev.tw1024 = b + off_t1k;
     pl->dev.twN = b + off_twN;
+    pl->dev.U = U; pl->dev.logM = ilog2(N * U);
+    pl->dev.twU = U > 1 ? b + off_twU : b + off_tw;
     pat->plans[key] = pl;
     *out = pl;
     return AERA_OK;
@@ -251,7 +256,7 @@ struct WsLayout {
 };
 
 // Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
-WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs, int n_stations)
+WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs, int n_stations, int n_patterns = 1, int upsample = 1)
 {
     const int k_hi = k_lo + K - 1;
     PlanDev band{}; band.N = N; band.k_lo = k_lo; band.k_hi = k_hi; band.K = K;
@@ -261,8 +266,8 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
     size_t per_dir = (size_t)K * 4 + 32;                                  // + 32: MINV_Q4 plane padding
     const size_t q32 = (size_t)128 * ((k_hi >> 5) - (k_lo >> 5) + 1);     // MINV_Q32 planes
     if (q32 > per_dir) per_dir = q32;
-    w.off_minv = o; o = align_up(o + (size_t)n_dirs * per_dir * cb);
-    size_t scratch = generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations);
+    w.off_minv = o; o = align_up(o + (size_t)n_patterns * n_dirs * per_dir * cb);   // one slab of n_dirs matrices per table
+    size_t scratch = generic_scratch_bytes(dtype, N, n_dirs * (long)n_stations, upsample);
     if (op != AERA_OP_SCAN && long_f32_supported(dtype, band) && long_f32_scratch_bytes(band) > scratch)
         scratch = long_f32_scratch_bytes(band);
     w.off_scratch = o; o = align_up(o + scratch);
@@ -447,12 +452,23 @@ size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dty
     return ws_layout(op, dtype, n_samples, k_lo, k_hi - k_lo + 1, n_events_or_dirs, n_stations).total;
 }
 
+// Options of the variants that share unfold_impl
+struct ImplExt {
+    const aera_pattern_t *const *patterns = nullptr; // several resident tables (aera_unfold_batch_multi) ...
+    int n_patterns = 1;
+    const int32_t *pattern_id = nullptr;             // ... and the antenna type of each station (device)
+    int input_i16 = 0;                               // traces are int16 ADC counts (aera_unfold_batch_i16)
+    double g0 = 1.0, g1 = 1.0;                       // volts per count of the two channels
+    int upsample = 1;                                // spectral up-sampling factor (aera_unfold_batch_upsampled)
+};
+
 // aera_unfold_batch (forward = 0) and aera_fold_batch (forward = 1: the same kernels with (1/N) H in place of
-// (1/N) H^-1, peaks into the workspace)
+// (1/N) H^-1, peaks into the workspace), and the multi-table / int16 / up-sampled variants through `ext`
 static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
                                  int n_samples, double fs_hz, const void *traces, const double *dirs,
                                  void *efield, void *peak_amp, int32_t *peak_idx,
-                                 void *workspace, size_t workspace_bytes, void *cuda_stream, int forward, int spec_mode = 0)
+                                 void *workspace, size_t workspace_bytes, void *cuda_stream, int forward, int spec_mode = 0,
+                                 const ImplExt &ext = ImplExt())
 {
     aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
     if (st != AERA_OK) return st;
@@ -465,10 +481,10 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
         return fail(AERA_ERR_INVALID_ARG, "dirs / peak_amp / peak_idx are not aligned to their element size");
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     Plan *pl = nullptr;
-    st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl);
+    st = get_plan(const_cast<aera_pattern *>(pattern), n_samples, fs_hz, s, &pl, ext.upsample);
     if (st != AERA_OK) return st;
     const WsLayout w = ws_layout(forward ? AERA_OP_FOLD : (spec_mode ? AERA_OP_RECONSTRUCT : AERA_OP_UNFOLD), dtype, n_samples,
-                                 pl->dev.k_lo, pl->dev.K, n_events, n_stations);
+                                 pl->dev.k_lo, pl->dev.K, n_events, n_stations, ext.n_patterns, ext.upsample);
     if (!workspace || misaligned(workspace, kAlign) || workspace_bytes < w.total)
         return fail(AERA_ERR_WORKSPACE, "workspace must be non-NULL, 256-byte aligned and >= %zu bytes (got %zu)", w.total, workspace_bytes);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
@@ -477,26 +493,40 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
         peak_idx = reinterpret_cast<int32_t *>(ws + w.off_peaks + (size_t)n_events * n_stations * 8);
     }
 
-    const bool warp_path = kernel_variant() == 0 && w32_supported(dtype, pl->dev);
-    const bool team_path = kernel_variant() == 0 && t4k_f64_supported(dtype, pl->dev);
-    const bool long_path = kernel_variant() == 0 && long_f32_supported(dtype, pl->dev);
-    // the warp and team kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
-    cudaError_t e = launch_minv(dtype, pattern->d_table, geom_of(pattern->desc), pl->dev, dirs, n_events, ws + w.off_minv,
-                                warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS)),
-                                ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples, s, forward);
+    // up-sampling runs on the generic kernels (the specialised ones transform on the input grid only)
+    const bool fast = kernel_variant() == 0 && ext.upsample == 1;
+    const bool warp_path = fast && w32_supported(dtype, pl->dev);
+    const bool team_path = fast && !ext.input_i16 && t4k_f64_supported(dtype, pl->dev);
+    const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
+    const int layout = warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS));
+    // complex elements of one event's matrices in this layout; the tables' slabs follow one another
+    const size_t per_event = layout == MINV_Q4 ? minv_q4_stride(pl->dev.k_lo, pl->dev.k_hi)
+                             : (layout == MINV_Q32 ? (size_t)128 * ((pl->dev.k_hi >> 5) - (pl->dev.k_lo >> 5) + 1) : (size_t)pl->dev.K * 4);
+    UnfoldExt x;
+    x.pattern_id = ext.pattern_id;
+    x.minv_pattern_stride = (size_t)n_events * per_event;
+    x.input_i16 = ext.input_i16;
+    // the warp, team and long kernels form 2 V_c, so their matrix carries 1/N instead of 2/N
+    const double scale = ((warp_path || team_path || long_path) ? 1.0 : 2.0) / (double)n_samples;
+    cudaError_t e = cudaSuccess;
+    for (int t = 0; t < ext.n_patterns && e == cudaSuccess; ++t) {
+        const aera_pattern_t *pt = ext.patterns ? ext.patterns[t] : pattern;
+        e = launch_minv(dtype, pt->d_table, geom_of(pt->desc), pl->dev, dirs, n_events,
+                        ws + w.off_minv + (size_t)t * x.minv_pattern_stride * cplx_bytes(dtype), layout, scale, s, forward, ext.g0, ext.g1);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
     note_kernel(warp_path ? "unfold_w32" : (team_path ? "unfold_t4k_f64" : (long_path ? "unfold_long_f32" : "generic")));
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s,
-                              spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode);
+                              spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode, x);
     else if (team_path)
-        e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s);
+        e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s, x);
     else if (long_path)
         e = launch_unfold_long_f32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv,
-                                   ws + w.off_scratch, s);
+                                   ws + w.off_scratch, s, x);
     else
         e = launch_unfold_generic(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx,
-                                  ws + w.off_minv, ws + w.off_scratch, s);
+                                  ws + w.off_minv, ws + w.off_scratch, s, x);
     if (e != cudaSuccess) return cuda_fail(e, "unfold kernel launch");
     return AERA_OK;
 }
@@ -517,6 +547,73 @@ aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_ev
     // the kernels read their "traces" argument and write their "efield" argument: swapped roles here
     return unfold_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, efield, dirs, traces, nullptr, nullptr,
                        workspace, workspace_bytes, cuda_stream, 1);
+}
+
+// ---- several tables, one antenna type per station
+static aera_status_t check_patterns(const aera_pattern_t *const *patterns, int n_patterns)
+{
+    if (!patterns || n_patterns < 1 || n_patterns > 64) return fail(AERA_ERR_INVALID_ARG, "patterns must be non-NULL and 1 <= n_patterns <= 64");
+    for (int t = 0; t < n_patterns; ++t) {
+        if (!patterns[t]) return fail(AERA_ERR_INVALID_ARG, "patterns[%d] is NULL", t);
+        const aera_pattern_desc_t &a = patterns[0]->desc, &b = patterns[t]->desc;
+        if (a.dtype != b.dtype) return fail(AERA_ERR_DTYPE_MISMATCH, "patterns[%d] has another dtype than patterns[0]", t);
+        if (a.n_freq != b.n_freq || a.freq0_hz != b.freq0_hz || a.dfreq_hz != b.dfreq_hz)
+            return fail(AERA_ERR_INVALID_ARG, "patterns[%d] has another frequency axis than patterns[0] (the in-band bins must agree)", t);
+    }
+    return AERA_OK;
+}
+
+size_t aera_workspace_bytes_ex(aera_op_t op, const aera_pattern_t *pattern, int dtype, long n_events_or_dirs,
+                               int n_stations, int n_samples, double fs_hz, int n_patterns, int upsample)
+{
+    if (op != AERA_OP_UNFOLD && op != AERA_OP_SCAN && op != AERA_OP_FOLD && op != AERA_OP_RECONSTRUCT) { fail(AERA_ERR_INVALID_ARG, "unknown op %d", (int)op); return 0; }
+    if (check_common(pattern, dtype, n_stations, n_samples, fs_hz) != AERA_OK) return 0;
+    if (n_events_or_dirs < 0 || n_patterns < 1 || n_patterns > 64) { fail(AERA_ERR_INVALID_ARG, "negative count or n_patterns outside 1..64"); return 0; }
+    if (upsample < 1 || (upsample & (upsample - 1)) != 0 || (long)upsample * n_samples > 65536) { fail(AERA_ERR_INVALID_ARG, "upsample=%d must be a power of two with upsample * n_samples <= 65536", upsample); return 0; }
+    int k_lo, k_hi;
+    if (compute_band(pattern->desc, n_samples, fs_hz, &k_lo, &k_hi) != AERA_OK) return 0;
+    return ws_layout(op, dtype, n_samples, k_lo, k_hi - k_lo + 1, n_events_or_dirs, n_stations, n_patterns, upsample).total;
+}
+
+aera_status_t aera_unfold_batch_multi(const aera_pattern_t *const *patterns, int n_patterns, const int32_t *pattern_id,
+                                      int dtype, int n_events, int n_stations, int n_samples, double fs_hz,
+                                      const void *traces, const double *dirs, void *efield, void *peak_amp, int32_t *peak_idx,
+                                      void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    aera_status_t st = check_patterns(patterns, n_patterns);
+    if (st != AERA_OK) return st;
+    if (!pattern_id || misaligned(pattern_id, 4)) return fail(AERA_ERR_INVALID_ARG, "pattern_id must be a non-NULL, 4-byte aligned device pointer");
+    ImplExt ext;
+    ext.patterns = patterns; ext.n_patterns = n_patterns; ext.pattern_id = pattern_id;
+    return unfold_impl(patterns[0], dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs, efield, peak_amp, peak_idx,
+                       workspace, workspace_bytes, cuda_stream, 0, 0, ext);
+}
+
+// ---- int16 ADC-count input, spectral up-sampling
+aera_status_t aera_unfold_batch_i16(const aera_pattern_t *pattern, int n_events, int n_stations, int n_samples, double fs_hz,
+                                    const int16_t *traces, const double *counts_to_volts, const double *dirs,
+                                    float *efield, float *peak_amp, int32_t *peak_idx,
+                                    void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!counts_to_volts || !std::isfinite(counts_to_volts[0]) || !std::isfinite(counts_to_volts[1]))
+        return fail(AERA_ERR_INVALID_ARG, "counts_to_volts must point to two finite factors (host memory)");
+    ImplExt ext;
+    ext.input_i16 = 1; ext.g0 = counts_to_volts[0]; ext.g1 = counts_to_volts[1];
+    return unfold_impl(pattern, AERA_F32, n_events, n_stations, n_samples, fs_hz, traces, dirs, efield, peak_amp, peak_idx,
+                       workspace, workspace_bytes, cuda_stream, 0, 0, ext);
+}
+
+aera_status_t aera_unfold_batch_upsampled(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations, int n_samples,
+                                          double fs_hz, int upsample, const void *traces, const double *dirs,
+                                          void *efield, void *peak_amp, int32_t *peak_idx,
+                                          void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (upsample < 1 || (upsample & (upsample - 1)) != 0 || (long)upsample * n_samples > 65536)
+        return fail(AERA_ERR_INVALID_ARG, "upsample=%d must be a power of two with upsample * n_samples <= 65536", upsample);
+    ImplExt ext;
+    ext.upsample = upsample;
+    return unfold_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces, dirs, efield, peak_amp, peak_idx,
+                       workspace, workspace_bytes, cuda_stream, 0, 0, ext);
 }
 
 aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int n_stations, int n_samples,

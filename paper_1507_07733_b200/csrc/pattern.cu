@@ -92,7 +92,7 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restrict__ dirs,
             const int *__restrict__ bin_if, const double *__restrict__ bin_tf, const double *__restrict__ bin_w, int K, double scale0,
-            int layout, int k_lo, int forward, cx<T> *__restrict__ minv)
+            int layout, int k_lo, int forward, cx<T> *__restrict__ minv, double g0, double g1)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
@@ -147,10 +147,11 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         cx<T> *o = minv + ((size_t)d * K + j) * 4;
         // E_theta = ( h3 V0 - h1 V1)/det ; E_phi = (-h2 V0 + h0 V1)/det
         cx<T> mt0, mt1, mp0, mp1; // theta <- V0, theta <- V1, phi <- V0, phi <- V1
-        mt0.re = (T)(hr[3] * ir - hi[3] * ii);    mt0.im = (T)(hr[3] * ii + hi[3] * ir);
-        mt1.re = (T)(-(hr[1] * ir - hi[1] * ii)); mt1.im = (T)(-(hr[1] * ii + hi[1] * ir));
-        mp0.re = (T)(-(hr[2] * ir - hi[2] * ii)); mp0.im = (T)(-(hr[2] * ii + hi[2] * ir));
-        mp1.re = (T)(hr[0] * ir - hi[0] * ii);    mp1.im = (T)(hr[0] * ii + hi[0] * ir);
+        // (g0, g1: per-channel input scale, e.g. volts per ADC count of int16 traces: V_c = g_c * raw_c, folded into the columns)
+        mt0.re = (T)(g0 * (hr[3] * ir - hi[3] * ii));    mt0.im = (T)(g0 * (hr[3] * ii + hi[3] * ir));
+        mt1.re = (T)(-g1 * (hr[1] * ir - hi[1] * ii)); mt1.im = (T)(-g1 * (hr[1] * ii + hi[1] * ir));
+        mp0.re = (T)(-g0 * (hr[2] * ir - hi[2] * ii)); mp0.im = (T)(-g0 * (hr[2] * ii + hi[2] * ir));
+        mp1.re = (T)(g1 * (hr[0] * ir - hi[0] * ii));    mp1.im = (T)(g1 * (hr[0] * ii + hi[0] * ir));
         if (forward) { // the forward model (aera_fold_batch): scale * H itself, rows (V0 <- E_theta, V0 <- E_phi, V1 <- E_theta, V1 <- E_phi)
             mt0.re = (T)(scale * hr[0]); mt0.im = (T)(scale * hi[0]); mt1.re = (T)(scale * hr[1]); mt1.im = (T)(scale * hi[1]);
             mp0.re = (T)(scale * hr[2]); mp0.im = (T)(scale * hi[2]); mp1.re = (T)(scale * hr[3]); mp1.im = (T)(scale * hi[3]);
@@ -183,7 +184,8 @@ size_t minv_smem_bytes(int dtype, int n_f)
 }
 
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
-                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s, int forward)
+                        const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s, int forward,
+                        double g0, double g1)
 {
     if (n_dirs <= 0) return cudaSuccess;
     ProfScope prof(KID_MINV, s);
@@ -192,11 +194,11 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
     if (dtype == AERA_F32) {
         AERA_ENSURE_DYN_SMEM(minv_kernel<float>, smem);
         minv_kernel<float><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<float> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
-                                                             p.K, scale, layout, p.k_lo, forward, (cx<float> *)minv);
+                                                             p.K, scale, layout, p.k_lo, forward, (cx<float> *)minv, g0, g1);
     } else {
         AERA_ENSURE_DYN_SMEM(minv_kernel<double>, smem);
         minv_kernel<double><<<(unsigned)n_dirs, 128, smem, s>>>((const cx<double> *)table, g, dirs, p.bin_if, p.bin_tf, forward ? nullptr : p.bin_w,
-                                                              p.K, scale, layout, p.k_lo, forward, (cx<double> *)minv);
+                                                              p.K, scale, layout, p.k_lo, forward, (cx<double> *)minv, g0, g1);
     }
     count_launches(1);
     return cudaGetLastError();

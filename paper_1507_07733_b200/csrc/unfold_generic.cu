@@ -101,11 +101,13 @@ __device__ __forceinline__ void zero_buffers(cx<T> *B, cx<T> *C, int N)
 }
 
 // a5 + a6 on buffers B (theta) and C (phi) holding the bit-reversed one-sided spectra.
+// With spectral up-sampling (p.U > 1) the buffers hold M = U N points and the transform is the inverse DFT of
+// length M of the same (zero-padded) spectrum: z[n] on a grid U times finer (aera_unfold_batch_upsampled).
 template <typename T>
 __device__ void inverse_and_peak(cx<T> *B, cx<T> *C, const PlanDev &p, T *ef, T *amp, int32_t *idx)
 {
-    const int N = p.N;
-    cta_fft<T, true, 2>(B, C, N, p.logN, (const cx<T> *)p.tw);
+    const int N = p.N * p.U;
+    cta_fft<T, true, 2>(B, C, N, p.logM, (const cx<T> *)p.twU);
     T best = (T)-1; int bi = 0x7fffffff;
     for (int n = threadIdx.x; n < N; n += blockDim.x) {
         cx<T> zt = B[n], zp = C[n];
@@ -116,13 +118,14 @@ __device__ void inverse_and_peak(cx<T> *B, cx<T> *C, const PlanDev &p, T *ef, T 
     cta_argmax<T>(best, bi, amp, idx);
 }
 
-template <typename T>
-__device__ void forward_spectrum(cx<T> *A, const PlanDev &p, const T *v)
+// IN = T, or int16_t for ADC-count input (the counts-to-volts factors are in Minv)
+template <typename T, typename IN>
+__device__ void forward_spectrum(cx<T> *A, const PlanDev &p, const IN *v)
 {
     const int N = p.N, sh = 32 - p.logN;
     for (int n = threadIdx.x; n < N; n += blockDim.x) {
         const int r = (int)(__brev((unsigned)n) >> sh);
-        A[r].re = v[n]; A[r].im = v[N + n];
+        A[r].re = (T)v[n]; A[r].im = (T)v[N + n];
     }
     __syncthreads();
     cta_fft<T, false, 1>(A, nullptr, N, p.logN, (const cx<T> *)p.tw);
@@ -145,32 +148,33 @@ __device__ __forceinline__ void apply_minv(const cx<T> *__restrict__ M, cx<T> v0
     ep.re = a.re + b.re; ep.im = a.im + b.im;
 }
 
-template <typename T, bool SMEM>
+template <typename T, bool SMEM, typename IN>
 __global__ void __launch_bounds__(kThreads)
-unfold_generic_kernel(PlanDev p, long n_units, int n_stations, const T *__restrict__ traces, T *efield,
+unfold_generic_kernel(PlanDev p, long n_units, int n_stations, const IN *__restrict__ traces, T *efield,
                       T *__restrict__ amp, int32_t *__restrict__ idx, const cx<T> *__restrict__ minv,
-                      cx<T> *scratch)
+                      cx<T> *scratch, const int32_t *__restrict__ pattern_id, size_t minv_pattern_stride)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = p.N, sh = 32 - p.logN;
-    cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * 3 * N;
-    cx<T> *B = A + N, *C = B + N;
+    const int N = p.N, M_ = p.N * p.U, shM = 32 - p.logM;   // transform sizes: forward N, inverse M_ = U N
+    cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * (N + 2 * (size_t)M_);
+    cx<T> *B = A + N, *C = B + M_;
 
     for (long u = blockIdx.x; u < n_units; u += gridDim.x) {
         const long ev = u / n_stations;
-        zero_buffers(B, C, N);
-        forward_spectrum<T>(A, p, traces + (size_t)u * 2 * N); // ends with __syncthreads
-        const cx<T> *M = minv + (size_t)ev * p.K * 4;
+        zero_buffers(B, C, M_);
+        forward_spectrum<T, IN>(A, p, traces + (size_t)u * 2 * N); // ends with __syncthreads
+        // one Minv per (event, antenna type of the station) when several tables are resident
+        const cx<T> *M = minv + (pattern_id ? (size_t)pattern_id[u - ev * n_stations] * minv_pattern_stride : 0) + (size_t)ev * p.K * 4;
         for (int j = threadIdx.x; j < p.K; j += blockDim.x) {
             const int k = p.k_lo + j;
             cx<T> v0, v1, et, ep;
             split_channels(A[k], A[N - k], v0, v1);
             apply_minv(M + 4 * j, v0, v1, et, ep);
-            const int r = (int)(__brev((unsigned)k) >> sh);
+            const int r = (int)(__brev((unsigned)k) >> shM);    // bin k of the length-M_ spectrum (zero-padded above the band)
             B[r] = et; C[r] = ep;
         }
         __syncthreads();
-        inverse_and_peak<T>(B, C, p, efield ? efield + (size_t)u * 2 * N : nullptr, amp + u, idx + u);
+        inverse_and_peak<T>(B, C, p, efield ? efield + (size_t)u * 2 * M_ : nullptr, amp + u, idx + u);
     }
 }
 
@@ -184,7 +188,7 @@ scan_forward_generic_kernel(PlanDev p, int n_stations, const T *__restrict__ tra
     const int N = p.N;
     cx<T> *A = SMEM ? reinterpret_cast<cx<T> *>(smem_raw) : scratch + (size_t)blockIdx.x * 3 * N;
     for (int s = blockIdx.x; s < n_stations; s += gridDim.x) {
-        forward_spectrum<T>(A, p, traces + (size_t)s * 2 * N);
+        forward_spectrum<T, T>(A, p, traces + (size_t)s * 2 * N);
         for (int j = threadIdx.x; j < p.K; j += blockDim.x) {
             const int k = p.k_lo + j;
             cx<T> v0, v1;
@@ -225,7 +229,7 @@ scan_inverse_generic_kernel(PlanDev p, int n_stations, long n_pairs, const cx<T>
 }
 
 size_t elem_bytes(int dtype) { return dtype == AERA_F32 ? sizeof(cx<float>) : sizeof(cx<double>); }
-bool fits_smem(int dtype, int N) { return (size_t)3 * N * elem_bytes(dtype) <= kSmemBudget; }
+bool fits_smem(int dtype, int N, int U = 1) { return ((size_t)N + 2 * (size_t)N * U) * elem_bytes(dtype) <= kSmemBudget; }
 long generic_grid(long n_units) { return n_units < (long)sm_count() * 4 ? n_units : (long)sm_count() * 4; }
 
 template <typename K>
@@ -234,21 +238,23 @@ cudaError_t set_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-template <typename T>
+template <typename T, typename IN>
 cudaError_t launch_unfold_t(int dtype, const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield,
-                            void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
+                            void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s, const UnfoldExt &x)
 {
     ProfScope prof(KID_UNFOLD, s);
     const long grid = generic_grid(n_units);
-    if (fits_smem(dtype, p.N)) {
-        size_t smem = (size_t)3 * p.N * sizeof(cx<T>);
-        cudaError_t e = set_smem(unfold_generic_kernel<T, true>, smem);
+    if (fits_smem(dtype, p.N, p.U)) {
+        size_t smem = ((size_t)p.N + 2 * (size_t)p.N * p.U) * sizeof(cx<T>);
+        cudaError_t e = set_smem(unfold_generic_kernel<T, true, IN>, smem);
         if (e != cudaSuccess) return e;
-        unfold_generic_kernel<T, true><<<(unsigned)grid, kThreads, smem, s>>>(
-            p, n_units, n_stations, (const T *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, nullptr);
+        unfold_generic_kernel<T, true, IN><<<(unsigned)grid, kThreads, smem, s>>>(
+            p, n_units, n_stations, (const IN *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, nullptr,
+            x.pattern_id, x.minv_pattern_stride);
     } else {
-        unfold_generic_kernel<T, false><<<(unsigned)grid, kThreads, 0, s>>>(
-            p, n_units, n_stations, (const T *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, (cx<T> *)scratch);
+        unfold_generic_kernel<T, false, IN><<<(unsigned)grid, kThreads, 0, s>>>(
+            p, n_units, n_stations, (const IN *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, (cx<T> *)scratch,
+            x.pattern_id, x.minv_pattern_stride);
     }
     count_launches(1);
     return cudaGetLastError();
@@ -290,10 +296,10 @@ cudaError_t launch_scan_t(int dtype, const PlanDev &p, int n_stations, const voi
 
 } // namespace
 
-size_t generic_scratch_bytes(int dtype, int N, long n_units)
+size_t generic_scratch_bytes(int dtype, int N, long n_units, int upsample)
 {
-    if (fits_smem(dtype, N)) return 0;
-    return (size_t)generic_grid(n_units) * 3 * N * elem_bytes(dtype);
+    if (fits_smem(dtype, N, upsample)) return 0;
+    return (size_t)generic_grid(n_units) * ((size_t)N + 2 * (size_t)N * upsample) * elem_bytes(dtype);
 }
 
 size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations)
@@ -302,13 +308,16 @@ size_t generic_scan_spectra_bytes(int dtype, int K, int n_stations)
 }
 
 cudaError_t launch_unfold_generic(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces,
-                                  void *efield, void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
+                                  void *efield, void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s,
+                                  const UnfoldExt &x)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
+    if (x.input_i16)   // int16 ADC counts in, fp32 out
+        return launch_unfold_t<float, int16_t>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s, x);
     return dtype == AERA_F32
-               ? launch_unfold_t<float>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s)
-               : launch_unfold_t<double>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s);
+               ? launch_unfold_t<float, float>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s, x)
+               : launch_unfold_t<double, double>(dtype, p, n_units, n_stations, traces, efield, amp, idx, minv, scratch, s, x);
 }
 
 cudaError_t launch_scan_generic(int dtype, const PlanDev &p, int n_stations, const void *traces, long n_dirs,

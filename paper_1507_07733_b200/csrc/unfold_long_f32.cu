@@ -61,6 +61,8 @@ struct LongParams {
     long n_units;
     int n_stations;
     int k_lo, k_hi, K, C;  // C = (k_hi >> 5) - (k_lo >> 5) + 1
+    const int32_t *pattern_id;   // [n_stations] antenna type per station, or nullptr (one table)
+    size_t minv_pattern_stride;  // float4 elements between the Minv slabs of consecutive tables
 };
 
 // L2 residency: the scratch (<= 55 x 0.96 MB) must stay in the 126 MB L2 while 1 MB per station streams
@@ -229,7 +231,8 @@ unfold_long_f32_kernel(LongParams p)
     for (long u = cluster_id; u < p.n_units; u += n_clusters) {
         const float *v0 = p.traces + (size_t)u * 2 * kLN, *v1 = v0 + kLN;
         float *ef = HAS_EF ? p.efield + (size_t)u * 2 * kLN : nullptr;
-        const float4 *Mev = p.minv + (size_t)(u / p.n_stations) * 64 * C;
+        const long ev = u / p.n_stations;
+        const float4 *Mev = p.minv + (size_t)ev * 64 * C + (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
 
         // ---------------- phase 1: loads + 32-point transform over j' + twiddle -> Y
 #pragma unroll 1
@@ -450,7 +453,7 @@ static size_t long_stride(const PlanDev &p)
 size_t long_f32_scratch_bytes(const PlanDev &p) { return long_max_clusters() * long_stride(p); }
 
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                                   void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s)
+                                   void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s, const UnfoldExt &x)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
@@ -461,6 +464,7 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
     q.scratch = (unsigned char *)scratch; q.scratch_stride = long_stride(p);
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.C = (p.k_hi >> 5) - (p.k_lo >> 5) + 1;
+    q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride / 2;   // complex float -> float4 elements
     const size_t smem = 8192 + 4096 + 128 + (size_t)kLWarps * kXBytes;
     cudaError_t e;
     auto launch = [&](auto kern) -> cudaError_t {

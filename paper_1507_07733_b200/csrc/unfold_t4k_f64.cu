@@ -58,6 +58,8 @@ struct T4kParams {
     long n_units;
     int n_stations;
     int k_lo, k_hi, K;
+    const int32_t *pattern_id;   // [n_stations] antenna type per station, or nullptr (one table)
+    size_t minv_pattern_stride;  // double2 elements between the Minv slabs of consecutive tables
 };
 
 __device__ __forceinline__ void team_sync(int team)
@@ -183,7 +185,9 @@ unfold_t4k_f64_kernel(T4kParams p)
     for (long u = u0 + team; u < u1; u += kTeams) {
         const double *v = p.traces + (size_t)u * 2 * N;
         double *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
-        const double2 *M = p.minv + (size_t)(u / p.n_stations) * minv_q4_stride(p.k_lo, p.k_hi);
+        const long ev = u / p.n_stations;
+        const double2 *M = p.minv + (size_t)ev * minv_q4_stride(p.k_lo, p.k_hi) +
+                           (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
         if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(double));
 
         double P[32], Q[32];
@@ -452,7 +456,7 @@ bool t4k_f64_supported(int dtype, const PlanDev &p)
 }
 
 cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s)
+                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
@@ -461,6 +465,7 @@ cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_station
     q.traces = (const double *)traces; q.efield = (double *)efield; q.amp = (double *)amp; q.idx = idx;
     q.minv = (const double2 *)minv; q.tw1024 = (const double2 *)p.tw1024; q.twN = (const double2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
+    q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
     cudaError_t e = efield ? launch_t4k<4, 12, true>(q, s) : launch_t4k<4, 12, false>(q, s);
     count_launches(1);
     return e;

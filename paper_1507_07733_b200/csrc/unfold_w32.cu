@@ -56,7 +56,9 @@ namespace {
 constexpr int kSolveUnroll = AERA_SOLVE_UNROLL;   // band rows of separate_solve in flight together
 
 struct W32Params {
-    const float *traces;
+    const void *traces;    // float [n_units][2][2048], or int16 ADC counts of the same shape (IN16)
+    const int32_t *pattern_id; // [n_stations] antenna type per station, or nullptr (one table)
+    size_t minv_pattern_stride; // float4 elements between the Minv slabs of consecutive tables
     float *efield;
     float *amp;
     int32_t *idx;
@@ -152,7 +154,7 @@ __device__ __forceinline__ void solve_from_spectra(const float4 *sp, float4 *XV,
     }
 }
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC>
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC, bool IN16>
 __global__ void __launch_bounds__(W32Geom<K2LO, K2HI>::kWarps * 32, 1)
 unfold_w32_kernel(W32Params p)
 {
@@ -217,11 +219,16 @@ unfold_w32_kernel(W32Params p)
 
 #pragma unroll 1
         for (long u = first; u < hi; u += kWarps) {
-            const float *v = p.traces + (size_t)u * 4 * kM;
+            const float *v = static_cast<const float *>(p.traces) + (size_t)u * 4 * kM;
+            const int16_t *v16 = static_cast<const int16_t *>(p.traces) + (size_t)u * 4 * kM;
+            // several tables resident: this station's antenna type selects the Minv slab (read through L1/L2)
+            const float4 *MAu = (MINV_SMEM || p.pattern_id == nullptr) ? MA : MA + (size_t)p.pattern_id[u - e * S] * p.minv_pattern_stride;
+            const float4 *MBu = MAu + p.K;
             float *ef = HAS_EF ? p.efield + (size_t)u * 4 * kM : nullptr;
             float4 *sp = SPEC != 0 ? p.spectra + (size_t)u * G::kBandRows * 32 + lane : nullptr;
             if (AERA_PREFETCH_DIST > 0 && lane == 0 && u + AERA_PREFETCH_DIST * kWarps < u1) {
-                if (SPEC != 2) prefetch_l2_bulk(v + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(float));
+                if (SPEC != 2 && IN16) prefetch_l2_bulk(v16 + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(int16_t));
+                else if (SPEC != 2) prefetch_l2_bulk(v + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(float));
                 else prefetch_l2_bulk(p.spectra + (size_t)(u + kWarps) * G::kBandRows * 32, G::kBandRows * 32 * sizeof(float4));
             }
 
@@ -231,13 +238,19 @@ unfold_w32_kernel(W32Params p)
                 static_for<0, 32>([&](auto jc) {
                     constexpr int j = decltype(jc)::value;
                     if (AERA_W32_ABLATE & 4) { A[brev5(j)] = L::pack(lane * 0.5f, j); B[brev5(j)] = L::pack(j, lane); return; }
+                    if (IN16) { // two ADC counts per 32-bit word: (v[2m], v[2m+1]); the counts-to-volts factors are in Minv
+                        const int a = ld_stream_b32(v16 + 2 * (lane + 32 * j)), b = ld_stream_b32(v16 + 2 * kM + 2 * (lane + 32 * j));
+                        A[brev5(j)] = L::pack((float)(short)(a & 0xffff), (float)(a >> 16));
+                        B[brev5(j)] = L::pack((float)(short)(b & 0xffff), (float)(b >> 16));
+                        return;
+                    }
                     A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
                     B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
                 });
             } else {
                 // ---- the forward spectrum of this station was stored by an earlier call: a4 straight away
                 if (!minv_ready) { mbar_wait(&full[slot], parity); minv_ready = true; }
-                solve_from_spectra<G, MINV_SMEM>(sp, reinterpret_cast<float4 *>(X), MA, MB, p.k_lo, p.k_hi, lane, tstash);
+                solve_from_spectra<G, MINV_SMEM>(sp, reinterpret_cast<float4 *>(X), MAu, MBu, p.k_lo, p.k_hi, lane, tstash);
                 __syncwarp(); // the buffer becomes a transpose plane again
                 tmem_wait_st();
                 build_inverse_input<G, false>(B, A, TS, lane, tstash);
@@ -299,7 +312,7 @@ unfold_w32_kernel(W32Params p)
                     // ---- separate channels, fold the two polyphase halves, a4: E = Minv V, one band
                     // row per iteration (a rolled loop: 40 instructions instead of 19 x 45), E goes to
                     // this lane's tensor-memory columns and is read back twice (s = 0, 1)
-                    if (!(AERA_W32_ABLATE & 16)) separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MA, MB, p.k_lo, p.k_hi, lane, tstash, sp);
+                    if (!(AERA_W32_ABLATE & 16)) separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MAu, MBu, p.k_lo, p.k_hi, lane, tstash, sp);
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
                     // ---- a5: even samples  z[2m] = IFFT_1024(E): inverse roles, A = Im, B = Re
@@ -362,12 +375,12 @@ size_t w32_smem_bytes(int K)
     return (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)G::kWarps * G::kWarpBytes;
 }
 
-template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC>
+template <int K2LO, int K2HI, bool HAS_EF, bool MINV_SMEM, int SPEC, bool IN16 = false>
 cudaError_t launch_inst(const W32Params &q, cudaStream_t s)
 {
     using G = W32Geom<K2LO, K2HI>;
     const size_t smem = w32_smem_bytes<K2LO, K2HI, MINV_SMEM>(q.K);
-    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, SPEC>;
+    auto kern = unfold_w32_kernel<K2LO, K2HI, HAS_EF, MINV_SMEM, SPEC, IN16>;
     AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + G::kWarps - 1) / G::kWarps;
     if (grid > sm_count()) grid = sm_count();
@@ -390,18 +403,27 @@ size_t w32_spectra_bytes(const PlanDev &p, long n_units)
 }
 
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra, int spec_mode)
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra, int spec_mode,
+                              const UnfoldExt &x)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
     ProfScope prof(KID_UNFOLD, s);
     W32Params q;
-    q.traces = (const float *)traces; q.efield = (float *)efield; q.amp = (float *)amp; q.idx = idx;
+    q.traces = traces; q.efield = (float *)efield; q.amp = (float *)amp; q.idx = idx;
+    q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride / 2;   // complex float -> float4 elements
     q.spectra = (float4 *)spectra;
     q.minv = (const float4 *)minv; q.tw1024 = (const float2 *)p.tw1024; q.twN = (const float2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     cudaError_t e;
-    if ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) { // configs[1]: 30-80 MHz at fs = 180 MHz
+    const bool cfg1_rows = (p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28;   // configs[1]: 30-80 MHz at fs = 180 MHz
+    if (x.input_i16) {           // int16 ADC counts in (Minv staged per event; one table)
+        if (cfg1_rows) e = efield ? launch_inst<10, 28, true, true, 0, true>(q, s) : launch_inst<10, 28, false, true, 0, true>(q, s);
+        else e = efield ? launch_inst<0, 31, true, false, 0, true>(q, s) : launch_inst<0, 31, false, false, 0, true>(q, s);
+    } else if (x.pattern_id) {   // one Minv per (event, antenna type): read through L1/L2 instead of the per-event smem ring
+        if (cfg1_rows) e = efield ? launch_inst<10, 28, true, false, 0>(q, s) : launch_inst<10, 28, false, false, 0>(q, s);
+        else e = efield ? launch_inst<0, 31, true, false, 0>(q, s) : launch_inst<0, 31, false, false, 0>(q, s);
+    } else if (cfg1_rows) {
         if (spectra && spec_mode == 1) e = efield ? launch_inst<10, 28, true, true, 1>(q, s) : launch_inst<10, 28, false, true, 1>(q, s);
         else if (spectra && spec_mode == 2) e = efield ? launch_inst<10, 28, true, true, 2>(q, s) : launch_inst<10, 28, false, true, 2>(q, s);
         else e = efield ? launch_inst<10, 28, true, true, 0>(q, s) : launch_inst<10, 28, false, true, 0>(q, s);

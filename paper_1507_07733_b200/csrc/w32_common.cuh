@@ -24,6 +24,12 @@ __device__ __forceinline__ R ld_stream_b64(const void *p)
     asm volatile("ld.global.nc.L1::no_allocate.b64 %0, [%1];" : "=l"(r.v) : "l"(p));
     return r;
 }
+__device__ __forceinline__ int ld_stream_b32(const void *p)
+{
+    int r;
+    asm volatile("ld.global.nc.L1::no_allocate.b32 %0, [%1];" : "=r"(r) : "l"(p));
+    return r;
+}
 __device__ __forceinline__ float4 ld_nc_f4(const float4 *p)
 {
     float4 r;
