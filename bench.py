@@ -430,6 +430,8 @@ def main():
     ap.add_argument("--loop", type=int, default=0, help="config 1 only: time the device-resident reconstruction loop with this many iterations")
     ap.add_argument("--fold", action="store_true", help="time the on-device forward model (aera_fold_batch) on the config's shapes")
     ap.add_argument("--peaks", action="store_true", help="measure and print the device's ALU issue peaks (packed fp32, fp32, fp64) and exit")
+    ap.add_argument("--i16", action="store_true", help="int16 ADC-count input (aera_unfold_batch_i16): 24 584 algorithmic bytes per unit at configs[1]")
+    ap.add_argument("--patterns", type=int, default=1, help="number of resident antenna-pattern tables, stations assigned round-robin (aera_unfold_batch_multi)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -501,6 +503,24 @@ def main():
     def step():
         B.aera_unfold_batch(pat, d_tr, d_dirs, wl.fs_hz, efield=d_ef, peak_amp=d_amp, peak_idx=d_idx, workspace=ws, stream=stream)
 
+    variant_note = None
+    if args.i16:        # the same batch as int16 ADC counts (1/16 microvolt per count), fp32 out
+        assert wl.dtype == "f32", "--i16 needs an fp32 config"
+        g16 = (0.0625, 0.0625)
+        d_tr16 = torch.clamp(torch.round(d_tr / g16[0]), -32768, 32767).to(torch.int16)
+        variant_note = "int16 ADC-count input (aera_unfold_batch_i16)"
+
+        def step():  # noqa: F811
+            B.aera_unfold_batch_i16(pat, d_tr16, g16, d_dirs, wl.fs_hz, efield=d_ef, peak_amp=d_amp, peak_idx=d_idx, workspace=ws, stream=stream)
+    elif args.patterns > 1:   # several antenna types, stations assigned round-robin
+        pats = [pat] + [B.aera_pattern_upload(B.make_desc(wl.grid, dt_code), ai.pattern_table(wl.grid, wl.complex_dtype, seed=1507 + t)) for t in range(1, args.patterns)]
+        d_pid = (torch.arange(wl.n_stations, dtype=torch.int32, device="cuda") % args.patterns).contiguous()
+        ws = B.alloc_workspace(B.aera_workspace_bytes_ex(B.AERA_OP_UNFOLD, pat, dt_code, n_events, wl.n_stations, wl.n_samples, wl.fs_hz, args.patterns, 1))
+        variant_note = f"{args.patterns} resident pattern tables, pattern_id[station] = station % {args.patterns} (aera_unfold_batch_multi)"
+
+        def step():  # noqa: F811
+            B.aera_unfold_batch_multi(pats, d_pid, d_tr, d_dirs, wl.fs_hz, efield=d_ef, peak_amp=d_amp, peak_idx=d_idx, workspace=ws, stream=stream)
+
     def barrier():
         if world > 1:
             dist.barrier()
@@ -543,6 +563,8 @@ def main():
     # ---- roofline of the dominant kernel (batched unfold), live CUDA-event timing inside the library
     peak, peak_src = load_peaks()
     bytes_unit = algorithmic_bytes_per_unit(wl)
+    if args.i16:
+        bytes_unit = 2 * wl.n_samples * 2 + 2 * wl.n_samples * 4 + 8     # int16 in, fp32 out, peak
     k_avg_ms = k_ms / max(k_n, 1)
     achieved = n_units * bytes_unit / (k_avg_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
@@ -561,7 +583,7 @@ def main():
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and variant_note is None:
         ne_h = host_tr.shape[0]           # the whole batch, or the canonical host block of a batch tiled on the device
         dirs_h = host_dirs[:ne_h]
         out_ef = torch.empty(host_tr.shape, dtype=host_tr.dtype, pin_memory=True)
@@ -586,7 +608,7 @@ def main():
 
     # ---- CPU oracle baseline on the box's host cores (rank 0, N=1 only), bounded sample
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and variant_note is None:
         import oracle
         cores = oracle.num_threads()
         n_ev_s = {1: 32, 3: 16, 4: 1}[wl.config]
@@ -625,7 +647,8 @@ def main():
             "config": {"workload": f"BASELINE configs[{wl.config}] {wl.name}: {n_events} events x {wl.n_stations} stations x 2 ch x {wl.n_samples} {wl.dtype} per GPU",
                        "n_events": n_events, "n_stations": wl.n_stations, "n_samples": wl.n_samples, "fs_hz": wl.fs_hz,
                        "l2_policy": f"inputs+outputs {2 * d_tr.numel() * d_tr.element_size() / 1e9:.1f} GB per step >> 126 MB L2 (no flush needed)",
-                       "kernel_variant": "auto" if args.variant == 0 else "generic", "sharding": "events across ranks, no collective"},
+                       "kernel_variant": "auto" if args.variant == 0 else "generic", "sharding": "events across ranks, no collective",
+                       "api_variant": variant_note, "kernel": B.aera_last_kernel()},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "outputs_sane": sane, "strong_pulse_idx_within_3": ok_idx, "setup_s": round(t_setup, 1), "library": B.aera_version(),
         }

@@ -14,9 +14,14 @@
 //       two packed (theta, phi) pruned inverse transforms, env^2 running argmax, one 8-byte result.
 //       No trace output: the kernel is pure FP32-pipe work.
 //
-// Tiles are ordered station-group-major and split into 148 contiguous ranges, so a CTA reloads V at
-// most twice and all CTAs sweep the direction list in step (the Minv planes they fetch are L2 hits
-// for everyone but the first).
+// Tiles are ordered station-group-major and split into one contiguous range per CTA, so a CTA reloads V at
+// most twice. Each CTA then streams its own part of the direction list: the 134 MB of per-direction matrices
+// (configs[2]) do not fit the L2 next to each other, so they are read from DRAM once per station group
+// (measured: 4.06 GB per launch, 0.9 TB/s = 14 % of the HBM peak, L2 hit rate 3 %). That costs nothing here
+// (the kernel is bound by the FP32 pipe), and the L2-friendly orders tried in round 2 were SLOWER: direction
+// blocks of 55 MB swept by all station groups (177 M pairs/s), chunks of 4..32 tiles dealt round-robin so that
+// all CTAs work on the same few directions at the same time (178..188 M pairs/s) against 203 M pairs/s for this
+// order -- 31 CTAs fetching the same 55 KB at the same moment queue up on the same L2 slices.
 #include "w32_common.cuh"
 
 namespace aera {
