@@ -27,8 +27,7 @@
 namespace aera {
 namespace {
 
-constexpr int kScanStations = 4; // stations per tile
-constexpr int kScanDirs = 3;     // directions per tile
+constexpr int kScanStations = 4; // stations per tile; directions per tile: 3 (12 warps) when the tensor-memory columns allow, else 2
 
 struct ScanParams {
     const float *traces;   // [S][2][2048]
@@ -108,11 +107,13 @@ scan_fwd_w32_kernel(ScanParams p)
 template <int K2LO, int K2HI>
 struct ScanGeom {
     using G = W32Geom<K2LO, K2HI>;
-    static constexpr int kWarps = kScanStations * kScanDirs;     // 12: three warps per scheduler
     static constexpr int kVCols = 4 * G::kBandRows;              // this station's 2 V_c, 4 columns per band row
     static constexpr int kCols = 2 * kVCols;                     // + the stash of E (read back for the odd samples)
-    static constexpr int kColStride = 512 / kScanDirs;           // warps w, w+4, w+8 share one TMEM lane quarter
+    static constexpr int kDirs = 3 * kCols <= 512 ? 3 : 2;       // directions per tile: warps w, w+4(, w+8) share one TMEM lane quarter
+    static constexpr int kWarps = kScanStations * kDirs;         // 12 (three warps per scheduler) or 8
+    static constexpr int kColStride = 512 / kDirs;
     static_assert(kCols <= kColStride, "tensor-memory columns per warp");
+    static constexpr bool kAnyBand = K2LO == 0 && K2HI == 31;    // rows may lie wholly outside the band: clamp every Minv index
 };
 
 template <int K2LO, int K2HI>
@@ -122,6 +123,7 @@ scan_inv_w32_kernel(ScanParams p)
     using G = W32Geom<K2LO, K2HI>;
     using SG = ScanGeom<K2LO, K2HI>;
     constexpr int kWarps = SG::kWarps;
+    constexpr int kScanDirs = SG::kDirs;
     extern __shared__ __align__(128) unsigned char smem[];
     float2 *T = reinterpret_cast<float2 *>(smem);
     float2 *TS = T + 1024;
@@ -215,8 +217,8 @@ scan_inv_w32_kernel(ScanParams p)
                     else {
                         constexpr int r = k2 - G::kLo;
                         int j = lane + 32 * k2 - p.k_lo; // edge rows: V is zero outside the band, keep the read in range
-                        if (k2 == G::kLo) j = j < 0 ? 0 : j;
-                        if (k2 == G::kHi) j = j > p.K - 1 ? p.K - 1 : j;
+                        if (SG::kAnyBand || k2 == G::kLo) j = j < 0 ? 0 : j;
+                        if (SG::kAnyBand || k2 == G::kHi) j = j > p.K - 1 ? p.K - 1 : j;
                         const float4 m0 = MA[j], m1 = MB[j];
                         const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
                         float v0r, v0i, v1r, v1i;
@@ -293,44 +295,51 @@ scan_inv_w32_kernel(ScanParams p)
 
 bool scan_w32_supported(int dtype, const PlanDev &p)
 {
-    // the one band geometry instantiated: rows 10..28 (30-80 MHz at fs = 180 MHz, configs[2])
-    return dtype == AERA_F32 && p.N == 2 * kM && p.k_hi < kM && p.k_lo >= 1 && (p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28;
+    // rows 10..28 (30-80 MHz at fs = 180 MHz, configs[2]) have their own instantiation; <0, 31> serves any other band
+    return dtype == AERA_F32 && p.N == 2 * kM && p.k_hi < kM && p.k_lo >= 1;
 }
 
 size_t scan_w32_spectra_bytes(int n_stations)
 {
-    return (size_t)n_stations * W32Geom<10, 28>::kBandRows * 32 * sizeof(float4);
+    return (size_t)n_stations * 32 * 32 * sizeof(float4);   // room for all 32 rows (any band)
+}
+
+template <int K2LO, int K2HI>
+static cudaError_t launch_scan_inst(const ScanParams &q, cudaStream_t s)
+{
+    using G = W32Geom<K2LO, K2HI>;
+    using SG = ScanGeom<K2LO, K2HI>;
+    {
+        ProfScope prof(KID_SCAN_FWD, s);
+        const size_t smem = (size_t)kTabBytes + 4 * (size_t)G::kWarpBytes;
+        auto kern = scan_fwd_w32_kernel<K2LO, K2HI>;
+        AERA_ENSURE_DYN_SMEM(kern, smem);
+        kern<<<(unsigned)((q.n_stations + 3) / 4), 128, smem, s>>>(q);
+    }
+    {
+        ProfScope prof(KID_SCAN_INV, s);
+        const size_t slot = ((size_t)SG::kDirs * q.K * 32 + 127) & ~(size_t)127;
+        const size_t smem = (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)SG::kWarps * kXBytes;
+        auto kern = scan_inv_w32_kernel<K2LO, K2HI>;
+        AERA_ENSURE_DYN_SMEM(kern, smem);
+        const long n_tiles = (long)((q.n_stations + kScanStations - 1) / kScanStations) * ((q.n_dirs + SG::kDirs - 1) / SG::kDirs);
+        const long grid = n_tiles < sm_count() ? n_tiles : sm_count();
+        kern<<<(unsigned)grid, SG::kWarps * 32, smem, s>>>(q);
+    }
+    return cudaGetLastError();
 }
 
 cudaError_t launch_scan_w32(const PlanDev &p, int n_stations, const void *traces, long n_dirs, const void *minv,
                             void *amp, int32_t *idx, void *spectra, cudaStream_t s)
 {
     if (n_dirs <= 0 || n_stations <= 0) return cudaSuccess;
-    using G = W32Geom<10, 28>;
     ScanParams q;
     q.traces = (const float *)traces; q.spectra = (float4 *)spectra; q.minv = (const float4 *)minv;
     q.amp = (float *)amp; q.idx = idx; q.tw1024 = (const float2 *)p.tw1024; q.twN = (const float2 *)p.twN;
     q.n_dirs = n_dirs; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
-    cudaError_t e;
-    {
-        ProfScope prof(KID_SCAN_FWD, s);
-        const size_t smem = (size_t)kTabBytes + 4 * (size_t)G::kWarpBytes;
-        auto kern = scan_fwd_w32_kernel<10, 28>;
-        AERA_ENSURE_DYN_SMEM(kern, smem);
-        kern<<<(unsigned)((n_stations + 3) / 4), 128, smem, s>>>(q);
-    }
-    {
-        ProfScope prof(KID_SCAN_INV, s);
-        const size_t slot = ((size_t)kScanDirs * p.K * 32 + 127) & ~(size_t)127;
-        const size_t smem = (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)ScanGeom<10, 28>::kWarps * kXBytes;
-        auto kern = scan_inv_w32_kernel<10, 28>;
-        AERA_ENSURE_DYN_SMEM(kern, smem);
-        const long n_tiles = (long)((n_stations + kScanStations - 1) / kScanStations) * ((n_dirs + kScanDirs - 1) / kScanDirs);
-        const long grid = n_tiles < sm_count() ? n_tiles : sm_count();
-        kern<<<(unsigned)grid, ScanGeom<10, 28>::kWarps * 32, smem, s>>>(q);
-    }
+    const cudaError_t e = ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) ? launch_scan_inst<10, 28>(q, s) : launch_scan_inst<0, 31>(q, s);
     count_launches(2);
-    return cudaGetLastError();
+    return e;
 }
 
 } // namespace aera

@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(kTeams *kTeamThreads, 1)
 unfold_t4k_f64_kernel(T4kParams p)
 {
     constexpr int kRows = RHI - RLO + 1;            // band rows per thread
-    static_assert(kRows >= 1 && kRows <= 9, "band rows: K <= 1024 means at most 9 rows of 128 bins touch the band");
+    static_assert(kRows >= 1 && kRows <= 16, "band rows of 128 bins below N/2");
     constexpr int kMirLo = 31 - RHI, kMirHi = (32 - RLO) > 31 ? 31 : (32 - RLO); // rows holding some band bin's mirror
     constexpr int kMirRows = kMirHi - kMirLo + 1;
     static_assert(4 * kMirRows * 512 <= kRegionX, "mirror rows fit region X");
@@ -450,9 +450,8 @@ cudaError_t launch_t4k(const T4kParams &q, cudaStream_t s)
 
 bool t4k_f64_supported(int dtype, const PlanDev &p)
 {
-    // the one band geometry instantiated: rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3])
-    return dtype == AERA_F64 && p.N == 4096 && p.K <= 1024 && p.k_lo >= 1 && p.k_hi < 2048 &&
-           (p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12;
+    // rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3]) have their own instantiation; <0, 15> serves any other band
+    return dtype == AERA_F64 && p.N == 4096 && p.k_lo >= 1 && p.k_hi < 2048;
 }
 
 cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
@@ -466,7 +465,9 @@ cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_station
     q.minv = (const double2 *)minv; q.tw1024 = (const double2 *)p.tw1024; q.twN = (const double2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
-    cudaError_t e = efield ? launch_t4k<4, 12, true>(q, s) : launch_t4k<4, 12, false>(q, s);
+    cudaError_t e;
+    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) e = efield ? launch_t4k<4, 12, true>(q, s) : launch_t4k<4, 12, false>(q, s);
+    else e = efield ? launch_t4k<0, 15, true>(q, s) : launch_t4k<0, 15, false>(q, s);
     count_launches(1);
     return e;
 }

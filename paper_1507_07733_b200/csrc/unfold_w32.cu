@@ -397,9 +397,9 @@ bool w32_supported(int dtype, const PlanDev &p)
 
 size_t w32_spectra_bytes(const PlanDev &p, long n_units)
 {
-    // only the configs[1] band geometry has the spectrum-reuse instantiations
-    if (!((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28)) return 0;
-    return (size_t)n_units * W32Geom<10, 28>::kBandRows * 32 * sizeof(float4);
+    // rows 10..28 (configs[1]) store their 19 band rows, any other band all 32 rows
+    const int rows = ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) ? W32Geom<10, 28>::kBandRows : 32;
+    return (size_t)n_units * rows * 32 * sizeof(float4);
 }
 
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
@@ -427,7 +427,11 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
         if (spectra && spec_mode == 1) e = efield ? launch_inst<10, 28, true, true, 1>(q, s) : launch_inst<10, 28, false, true, 1>(q, s);
         else if (spectra && spec_mode == 2) e = efield ? launch_inst<10, 28, true, true, 2>(q, s) : launch_inst<10, 28, false, true, 2>(q, s);
         else e = efield ? launch_inst<10, 28, true, true, 0>(q, s) : launch_inst<10, 28, false, true, 0>(q, s);
-    } else
+    } else if (spectra && spec_mode == 1)
+        e = efield ? launch_inst<0, 31, true, false, 1>(q, s) : launch_inst<0, 31, false, false, 1>(q, s);
+    else if (spectra && spec_mode == 2)
+        e = efield ? launch_inst<0, 31, true, false, 2>(q, s) : launch_inst<0, 31, false, false, 2>(q, s);
+    else
         e = efield ? launch_inst<0, 31, true, false, 0>(q, s) : launch_inst<0, 31, false, false, 0>(q, s);
     count_launches(1);
     return e;
