@@ -338,7 +338,9 @@ def run_loop(args, wl):
     # the last iteration writes the E-field; 8 bytes of peaks per iteration and for the voltage timing
     spec = 19 * 32 * 16
     b_unit = 2 * wl.n_samples * 4 * 2 + spec * (1 + max(n_iter - 1, 0) if n_iter > 1 else 0) + 2 * wl.n_samples * 4 + 8 * (n_iter + 1)
-    achieved = n_units * b_unit / (ms_step * 1e-3) / 1e9
+    moved = n_units * b_unit / (ms_step * 1e-3) / 1e9      # bytes the design moves (second trace read, spectra spill and reloads included)
+    b_min = 2 * wl.n_samples * 4 * 2 + 8                    # minimal algorithmic bytes of one unit of the loop: traces read once, E-field written once, one peak
+    achieved = n_units * b_min / (ms_step * 1e-3) / 1e9
     dirs = out["r"]["dirs_hist"][-1].cpu().numpy()
     err = np.abs(np.sin(np.deg2rad(dirs[:, 0])) - np.sin(np.deg2rad(true_dirs[:, 0])))
     line = {
@@ -348,7 +350,8 @@ def run_loop(args, wl):
         "config": {"workload": f"BASELINE configs[1] shapes, reconstruction loop: {n_events} events x {wl.n_stations} stations x 2 ch x {wl.n_samples} f32, {n_iter} iterations",
                    "n_events": n_events, "n_iter": n_iter, "l2_policy": f"traces + E-field {2 * d_tr.numel() * 4 / 1e9:.1f} GB >> 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                     "kernel": "whole loop (timing + n_iter x (fit, Minv, unfold))", "algorithmic_bytes_per_unit": b_unit,
+                     "kernel": "whole loop (timing + n_iter x (fit, Minv, unfold))", "algorithmic_bytes_per_unit": b_min,
+                     "moved_bytes_per_unit": b_unit, "moved_gbs": moved, "moved_frac_of_peak": moved / peak,
                      "unfold_ms_mean": k_ms / max(k_n, 1), "timing_kernel_ms": t_ms / max(t_n, 1), "planefit_kernel_ms": f_ms / max(f_n, 1), "peak_source": peak_src},
         "cpu_baseline": None, "e2e": None, "gpu_launches": int(launches), "clocks": clocks,
         "outputs_sane": bool(np.isfinite(dirs).all() and np.median(err) < 0.02), "median_abs_err_sin_theta": float(np.median(err)),
@@ -576,7 +579,8 @@ def main():
     if os.path.exists(tpath):
         try:
             roofline["traffic"] = float(json.load(open(tpath))["dram_bytes_per_unit"]) * n_units
-            roofline["traffic_source"] = f"profiles/traffic_config{wl.config}.txt (ncu dram__bytes_read+write per unit x units per launch)"
+            roofline["traffic_source"] = (f"STATIC: profiles/traffic_config{wl.config}.txt (one committed ncu --set full capture, dram__bytes_read+write "
+                                          "per unit x units per launch); not measured in this run")
         except Exception:
             pass
     roofline["algorithmic_bytes_per_launch"] = n_units * bytes_unit

@@ -256,6 +256,17 @@ aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, i
                                      int32_t *idx0, void *w0, void *workspace, size_t workspace_bytes,
                                      void *cuda_stream);
 
+/* Convergence of the reconstruction loop (section 2: "On convergence, the timing information yields the
+ * incident direction of the primary particle"; the paper gives no criterion, reading R21): for every event the
+ * first iteration it >= 1 whose fitted direction lies within tol_deg (angle on the unit sphere, degrees) of iteration
+ * it - 1, or -1 if none does. The caller runs aera_reconstruct_batch with an upper bound n_iter and reads the direction
+ * and peaks of iteration conv_iter[event] (or the last one).
+ *   dirs_hist  DEVICE [n_iter][n_events][2] double, as written by aera_reconstruct_batch
+ *   conv_iter  DEVICE [n_events] int32, out
+ * Asynchronous on the stream. Errors: INVALID_ARG, CUDA. */
+aera_status_t aera_reconstruct_convergence(const double *dirs_hist, int n_iter, int n_events, double tol_deg,
+                                           int32_t *conv_iter, void *cuda_stream);
+
 /* End-to-end convenience for HOST buffers (the paper's situation: traces live on
  * the host and are copied for every transform).  Same arguments as aera_unfold_batch but every
  * data pointer is a HOST pointer (page-locked memory gives full PCIe speed; pageable works).

@@ -67,3 +67,22 @@ def reconstruct_event(grid, H, fs_hz: float, traces, positions, n_iter: int):
         t, w = last["idx"].astype(np.float64), last["amp"] ** 2
     return dict(idx0=idx0, w0=w0, dirs=np.array(dirs), amp=np.array(amps), idx=np.array(idxs),
                 efield=last["efield"] if last is not None else None)
+
+
+def angular_distance_deg(d0, d1):
+    """Angle between two arrival directions (theta, phi in degrees) on the unit sphere, in degrees."""
+    t0, p0, t1, p1 = np.radians([d0[0], d0[1], d1[0], d1[1]])
+    a = np.array([np.sin(t0) * np.cos(p0), np.sin(t0) * np.sin(p0), np.cos(t0)])
+    b = np.array([np.sin(t1) * np.cos(p1), np.sin(t1) * np.sin(p1), np.cos(t1)])
+    return float(np.degrees(np.arctan2(np.linalg.norm(np.cross(a, b)), np.dot(a, b))))
+
+
+def convergence_iteration(dirs, tol_deg: float) -> int:
+    """"On convergence, the timing information yields the incident direction ...". The paper gives no
+    criterion (reading R21): the loop has converged at the first iteration it >= 1 whose fitted direction lies
+    within tol_deg (angle on the sphere) of the previous iteration's; -1 if none does. dirs [n_iter][2] degrees."""
+    d = np.asarray(dirs, dtype=np.float64)
+    for it in range(1, len(d)):
+        if angular_distance_deg(d[it - 1], d[it]) < tol_deg:
+            return it
+    return -1

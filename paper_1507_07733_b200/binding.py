@@ -22,7 +22,7 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel", "aera_unfold_batch_multi", "aera_unfold_batch_i16",
-           "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex")
+           "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex", "aera_reconstruct_convergence")
 
 
 class AeraError(RuntimeError):
@@ -91,6 +91,8 @@ def _load():
     lib.aera_unfold_batch_upsampled.restype = C.c_int
     lib.aera_workspace_bytes_ex.argtypes = [C.c_int, vp, C.c_int, C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int]
     lib.aera_workspace_bytes_ex.restype = C.c_size_t
+    lib.aera_reconstruct_convergence.argtypes = [dp, C.c_int, C.c_int, C.c_double, vp, vp]
+    lib.aera_reconstruct_convergence.restype = C.c_int
     lib.aera_last_kernel.restype = C.c_char_p
     lib.aera_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), ip, ip]
     lib.aera_measure_alu_peak.restype = C.c_int
@@ -381,6 +383,15 @@ def aera_reconstruct_batch(p: Pattern, traces: torch.Tensor, positions: torch.Te
                                        _ptr(efield) if efield is not None else None, _ptr(amp_hist), _ptr(idx_hist), _ptr(idx0), _ptr(w0),
                                        _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
     return dict(dirs_hist=dirs_hist, efield=efield, amp_hist=amp_hist, idx_hist=idx_hist, idx0=idx0, w0=w0)
+
+
+def aera_reconstruct_convergence(dirs_hist: torch.Tensor, tol_deg: float, stream=None) -> torch.Tensor:
+    """dirs_hist [n_iter][E][2] CUDA float64 -> conv_iter [E] int32 (first iteration within tol_deg of its predecessor, else -1)."""
+    n_iter, E, two = dirs_hist.shape
+    assert two == 2 and dirs_hist.is_cuda and dirs_hist.dtype == torch.float64 and dirs_hist.is_contiguous()
+    out = torch.empty((E,), dtype=torch.int32, device=dirs_hist.device)
+    _check(_lib.aera_reconstruct_convergence(_ptr(dirs_hist), n_iter, E, float(tol_deg), _ptr(out), _stream_ptr(stream)))
+    return out
 
 
 def aera_unfold_batch_host(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, efield=None, peak_amp=None,

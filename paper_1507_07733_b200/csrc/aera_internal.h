@@ -129,6 +129,8 @@ cudaError_t launch_timing(int dtype, const void *traces, long n_units, int N, in
 cudaError_t launch_planefit(int dtype, const double *pos, const int32_t *idx, const void *w, int square_w, long n_events,
                             int n_stations, double fs, double *dirs, cudaStream_t s);
 
+cudaError_t launch_convergence(const double *dirs_hist, int n_iter, long n_events, double tol_deg, int32_t *conv_iter, cudaStream_t s);
+
 // ---- scan_w32.cu: direction scan for N = 2048 fp32, band rows 10..28 (configs[2])
 bool scan_w32_supported(int dtype, const PlanDev &p);
 size_t scan_w32_spectra_bytes(int n_stations);

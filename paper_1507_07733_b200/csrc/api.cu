@@ -109,7 +109,8 @@ struct aera_pattern {
     aera_pattern_desc_t desc{};
     void *d_table = nullptr;
     size_t table_bytes = 0;
-    std::mutex mu;
+    std::mutex mu;        // plans and filter weights
+    std::mutex pipe_mu;   // the host pipeline's staging buffers and streams: one aera_unfold_batch_host at a time per handle
     std::map<std::pair<long long, double>, Plan *> plans;   // key: (n_samples | up-sampling factor << 32, fs)
     HostPipe pipe;
 };
@@ -423,8 +424,11 @@ aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_sample
     Plan *pl = nullptr;
     st = get_plan(pattern, n_samples, fs_hz, s, &pl);
     if (st != AERA_OK) return st;
-    cudaError_t e = cudaStreamSynchronize(s); // no kernel of an earlier call may still read the old weights
-    if (e != cudaSuccess) return cuda_fail(e, "stream synchronise");
+    // a configuration call: no kernel of an earlier call on ANY stream (the host pipeline has its own) may still read the
+    // old weights, and no other thread may build or fetch a plan of this pattern meanwhile
+    std::lock_guard<std::mutex> lk(pattern->mu);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(e, "device synchronise");
     if (!weights) { cudaFree(pl->d_filter); pl->d_filter = nullptr; pl->dev.bin_w = nullptr; return AERA_OK; }
     if (n_weights != pl->dev.K)
         return fail(AERA_ERR_INVALID_ARG, "n_weights=%d but the band of (n_samples=%d, fs=%g) has %d bins (aera_band)", n_weights, n_samples, fs_hz, pl->dev.K);
@@ -701,6 +705,15 @@ aera_status_t aera_reconstruct_batch(const aera_pattern_t *pattern, int dtype, i
     return AERA_OK;
 }
 
+aera_status_t aera_reconstruct_convergence(const double *dirs_hist, int n_iter, int n_events, double tol_deg, int32_t *conv_iter, void *cuda_stream)
+{
+    if (!dirs_hist || !conv_iter) return fail(AERA_ERR_INVALID_ARG, "dirs_hist and conv_iter must be non-NULL");
+    if (n_iter < 1 || n_events < 0 || !(tol_deg > 0)) return fail(AERA_ERR_INVALID_ARG, "n_iter >= 1, n_events >= 0 and tol_deg > 0 are required");
+    cudaError_t e = launch_convergence(dirs_hist, n_iter, n_events, tol_deg, conv_iter, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "convergence kernel launch");
+    return AERA_OK;
+}
+
 aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
                                      int n_samples, double fs_hz, const void *traces_host,
                                      const double *dirs_host, void *efield_host, void *peak_amp_host,
@@ -721,8 +734,11 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
     if (chunk_events < 1) chunk_events = 1;
     if (chunk_events > n_events) chunk_events = n_events;
 
+    std::lock_guard<std::mutex> pipe_lock(pattern->pipe_mu);
     HostPipe &hp = pattern->pipe;
     cudaError_t e;
+    // every error exit below first drains the three streams: no copy into the caller's buffers may be in flight on return
+    auto drained = [&](aera_status_t st_) { for (int i = 0; i < 3; ++i) if (hp.st[i]) cudaStreamSynchronize(hp.st[i]); return st_; };
     if (!hp.ready) {
         for (int i = 0; i < 3; ++i) { e = cudaStreamCreateWithFlags(&hp.st[i], cudaStreamNonBlocking); if (e != cudaSuccess) return cuda_fail(e, "stream create"); }
         for (int i = 0; i < 2; ++i) {
@@ -762,22 +778,22 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
         // stage b's input buffer is free once the kernel that read it (2 iterations ago) finished;
         // its output buffers are free once their D2H copy finished.
         if (it >= 2) {
-            if ((e = cudaStreamWaitEvent(hp.st[0], hp.ev_k[b], 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
-            if ((e = cudaStreamWaitEvent(hp.st[1], hp.ev_out[b], 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
+            if ((e = cudaStreamWaitEvent(hp.st[0], hp.ev_k[b], 0)) != cudaSuccess) return drained(cuda_fail(e, "stream wait"));
+            if ((e = cudaStreamWaitEvent(hp.st[1], hp.ev_out[b], 0)) != cudaSuccess) return drained(cuda_fail(e, "stream wait"));
         }
-        if ((e = cudaMemcpyAsync(hp.d_in[b], tin + (size_t)done * event_bytes, (size_t)ne * event_bytes, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return cuda_fail(e, "H2D traces");
-        if ((e = cudaMemcpyAsync(hp.d_dirs[b], dirs_host + 2 * done, (size_t)ne * 16, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return cuda_fail(e, "H2D dirs");
+        if ((e = cudaMemcpyAsync(hp.d_in[b], tin + (size_t)done * event_bytes, (size_t)ne * event_bytes, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return drained(cuda_fail(e, "H2D traces"));
+        if ((e = cudaMemcpyAsync(hp.d_dirs[b], dirs_host + 2 * done, (size_t)ne * 16, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return drained(cuda_fail(e, "H2D dirs"));
         cudaEventRecord(hp.ev_in[b], hp.st[0]);
         cudaStreamWaitEvent(hp.st[1], hp.ev_in[b], 0);
         st = aera_unfold_batch(pattern, dtype, (int)ne, n_stations, n_samples, fs_hz, hp.d_in[b], hp.d_dirs[b],
                                efield_host ? hp.d_out[b] : nullptr, hp.d_amp[b], hp.d_idx[b], hp.d_ws[b], hp.cap_ws, hp.st[1]);
-        if (st != AERA_OK) { cudaDeviceSynchronize(); return st; }
+        if (st != AERA_OK) return drained(st);
         cudaEventRecord(hp.ev_k[b], hp.st[1]);
         cudaStreamWaitEvent(hp.st[2], hp.ev_k[b], 0);
         if (efield_host)
-            if ((e = cudaMemcpyAsync(eout + (size_t)done * event_bytes, hp.d_out[b], (size_t)ne * event_bytes, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H efield");
-        if ((e = cudaMemcpyAsync(aout + (size_t)done * n_stations * rb, hp.d_amp[b], units * rb, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H amp");
-        if ((e = cudaMemcpyAsync(peak_idx_host + (size_t)done * n_stations, hp.d_idx[b], units * 4, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return cuda_fail(e, "D2H idx");
+            if ((e = cudaMemcpyAsync(eout + (size_t)done * event_bytes, hp.d_out[b], (size_t)ne * event_bytes, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return drained(cuda_fail(e, "D2H efield"));
+        if ((e = cudaMemcpyAsync(aout + (size_t)done * n_stations * rb, hp.d_amp[b], units * rb, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return drained(cuda_fail(e, "D2H amp"));
+        if ((e = cudaMemcpyAsync(peak_idx_host + (size_t)done * n_stations, hp.d_idx[b], units * 4, cudaMemcpyDeviceToHost, hp.st[2])) != cudaSuccess) return drained(cuda_fail(e, "D2H idx"));
         cudaEventRecord(hp.ev_out[b], hp.st[2]);
         done += ne; ++it;
     }

@@ -107,7 +107,37 @@ planefit_kernel(const double *__restrict__ pos, const int32_t *__restrict__ idx,
     if (lane == 0) { dirs[2 * e] = theta; dirs[2 * e + 1] = phi; }
 }
 
+// first iteration it >= 1 whose direction lies within tol_deg (angle on the sphere) of the previous one, else -1
+__global__ void convergence_kernel(const double *__restrict__ dirs_hist, int n_iter, long n_events, double tol_deg, int32_t *__restrict__ conv_iter)
+{
+    const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_events) return;
+    const double d2r = 3.14159265358979323846 / 180.0;
+    int found = -1;
+    double st, ct, sp, cp;
+    sincos(dirs_hist[2 * e] * d2r, &st, &ct); sincos(dirs_hist[2 * e + 1] * d2r, &sp, &cp);
+    double ax = st * cp, ay = st * sp, az = ct;
+    for (int it = 1; it < n_iter; ++it) {
+        const double *d = dirs_hist + ((size_t)it * n_events + e) * 2;
+        sincos(d[0] * d2r, &st, &ct); sincos(d[1] * d2r, &sp, &cp);
+        const double bx = st * cp, by = st * sp, bz = ct;
+        const double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;
+        const double ang = atan2(sqrt(cx * cx + cy * cy + cz * cz), ax * bx + ay * by + az * bz) / d2r;
+        if (found < 0 && ang < tol_deg) found = it;
+        ax = bx; ay = by; az = bz;
+    }
+    conv_iter[e] = found;
+}
+
 } // namespace
+
+cudaError_t launch_convergence(const double *dirs_hist, int n_iter, long n_events, double tol_deg, int32_t *conv_iter, cudaStream_t s)
+{
+    if (n_events <= 0) return cudaSuccess;
+    convergence_kernel<<<(unsigned)((n_events + 127) / 128), 128, 0, s>>>(dirs_hist, n_iter, n_events, tol_deg, conv_iter);
+    count_launches(1);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_timing(int dtype, const void *traces, long n_units, int N, int32_t *idx0, void *w0, cudaStream_t s)
 {

@@ -113,3 +113,22 @@ def test_spectrum_reuse_is_bit_identical(B):
             assert torch.equal(a[k], b[k]), k
     finally:
         pat.free()
+
+
+def test_reconstruct_convergence_matches_oracle(B):
+    from oracle import aera_loop as ol
+    rng = np.random.default_rng(8)
+    n_iter, E = 5, 300
+    d = np.empty((n_iter, E, 2))
+    d[0, :, 0] = rng.uniform(0, 80, E); d[0, :, 1] = rng.uniform(0, 360, E)
+    for it in range(1, n_iter):    # shrinking steps; some events jump across phi = 0 / 360, some sit at the zenith
+        d[it] = d[it - 1] + rng.normal(0, 1.0, (E, 2)) * 10.0 ** (-it * rng.uniform(0.3, 1.5, (E, 1)))
+        d[it, :, 1] %= 360.0
+    d[:, :5, 0] = 0.0
+    d[1:, 280:, 0] += rng.uniform(3, 10, (n_iter - 1, 20)).cumsum(axis=0)      # these never settle
+    d[:, :, 0] = np.clip(d[:, :, 0], 0, 85)
+    got = B.aera_reconstruct_convergence(torch.from_numpy(d).cuda(), 0.05).cpu().numpy()
+    ref = np.array([ol.convergence_iteration(d[:, e], 0.05) for e in range(E)])
+    # an angle within 1e-9 degree of the tolerance may fall on either side of it
+    near = np.array([any(abs(ol.angular_distance_deg(d[i - 1, e], d[i, e]) - 0.05) < 1e-9 for i in range(1, n_iter)) for e in range(E)])
+    assert np.array_equal(got[~near], ref[~near]) and set(np.unique(ref)) >= {-1, 1}

@@ -95,3 +95,15 @@ def test_loop_recovers_the_injected_direction_from_synthetic_traces(small_table)
     th0, ph0 = ev.direction_deg
     assert abs(th - th0) < 1.0 and abs((ph - ph0 + 180.0) % 360.0 - 180.0) < 2.0 / max(np.sin(np.deg2rad(th0)), 0.2)
     assert r["idx"].shape == (2, 40) and r["efield"].shape == (40, 2, wl.n_samples)
+
+
+def test_convergence_iteration_closed_forms():
+    """The angular distance is the great-circle angle (pole: azimuth irrelevant; equator: azimuth difference) and the
+    criterion picks the first iteration within tolerance of its predecessor."""
+    assert abs(ol.angular_distance_deg((0.0, 10.0), (0.0, 200.0))) < 1e-12            # both at the zenith
+    assert abs(ol.angular_distance_deg((90.0, 10.0), (90.0, 40.0)) - 30.0) < 1e-12    # along the horizon
+    assert abs(ol.angular_distance_deg((30.0, 77.0), (50.0, 77.0)) - 20.0) < 1e-12    # along a meridian
+    assert abs(ol.angular_distance_deg((30.0, 359.9), (30.0, 0.1)) - 0.2 * np.sin(np.radians(30.0))) < 1e-6
+    dirs = [(40.0, 100.0), (42.0, 101.0), (42.05, 101.0), (42.05, 101.0)]
+    assert ol.convergence_iteration(dirs, 0.1) == 2 and ol.convergence_iteration(dirs, 1e-9) == 3
+    assert ol.convergence_iteration(dirs[:2], 0.1) == -1 and ol.convergence_iteration(dirs, 5.0) == 1
