@@ -48,6 +48,17 @@ __device__ __forceinline__ unsigned long long tmem_ld64(uint32_t addr)
                  "tcgen05.ld.sync.aligned.32x32b.x2.b32 {lo, hi}, [%1];\nmov.b64 %0, {lo, hi};\n}" : "=l"(v) : "r"(addr) : "memory");
     return v;
 }
+// one 32-bit column per thread
+__device__ __forceinline__ uint32_t tmem_ld32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void tmem_ld_dep32(uint32_t &a, uint32_t &b)
+{
+    asm volatile("" : "+r"(a), "+r"(b) :: "memory");
+}
 // Results of earlier tmem_ld64 calls may be used only after tmem_wait_ld(). The compiler does not
 // know that, so each loaded value is then passed through tmem_ld_dep(): an empty volatile asm that
 // "rewrites" it. Volatile asms keep their order, so no consumer can be scheduled above the wait.

@@ -253,7 +253,7 @@ unfold_w32_kernel(W32Params p)
                 solve_from_spectra<G, MINV_SMEM>(sp, reinterpret_cast<float4 *>(X), MAu, MBu, p.k_lo, p.k_hi, lane, tstash);
                 __syncwarp(); // the buffer becomes a transpose plane again
                 tmem_wait_st();
-                build_inverse_input<G, false>(B, A, TS, lane, tstash);
+                build_inverse_input_eo<G>(B, A, TS, lane, tstash);
             }
 
             // ---- three 1024-point transforms through ONE copy of the FFT code (the instruction
@@ -311,21 +311,19 @@ unfold_w32_kernel(W32Params p)
                     if (!minv_ready) { mbar_wait(&full[slot], parity); minv_ready = true; }
                     // ---- separate channels, fold the two polyphase halves, a4: E = Minv V, one band
                     // row per iteration (a rolled loop: 40 instructions instead of 19 x 45), E goes to
-                    // this lane's tensor-memory columns and is read back twice (s = 0, 1)
+                    // this lane's tensor-memory columns and is read back once per polarisation
                     if (!(AERA_W32_ABLATE & 16)) separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MAu, MBu, p.k_lo, p.k_hi, lane, tstash, sp);
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
-                    // ---- a5: even samples  z[2m] = IFFT_1024(E): inverse roles, A = Im, B = Re
-                    build_inverse_input<G, false>(B, A, TS, lane, tstash);
-                } else {
-                    emit_even<HAS_EF>(B, A, tpark, best0, b0);
-                    // ---- odd samples  z[2m+1] = IFFT_1024(E W_2048^-k)
-                    build_inverse_input<G, true>(B, A, TS, lane, tstash);
-                    if (HAS_EF) tmem_wait_st(); // parked samples are in tensor memory before emit_odd reads them
-                }
+                } else
+                    emit_theta<HAS_EF>(B, A, lane, tpark, ef);
+                // ---- a5 (one copy of the code for both polarisations; the registers are dead at this join):
+                // (z[2m], z[2m+1]) = IFFT_1024 of (E_p, E_p W_2048^-k), p = theta after t = 0, phi after t = 1;
+                // inverse roles, A = Im, B = Re
+                build_inverse_input_eo<G>(B, A, TS, lane, tstash + (uint32_t)t);
                 ++t;
             }
-            emit_odd<HAS_EF>(B, A, lane, tpark, ef, best1, b1);
+            emit_phi<HAS_EF>(B, A, lane, tpark, ef, best0, b0, best1, b1);
 
             // ---- a6: lane result (lowest index on ties), then warp argmax with the same rule
             float best = best0; int bi = 2 * (lane + 32 * b0);

@@ -154,6 +154,84 @@ __device__ __forceinline__ void emit_odd(const R (&zr)[32], const R (&zi)[32], i
     });
 }
 
+// ---- (even, odd) sample packing: the two halves of a packed register carry z[2m] and z[2m+1] of ONE polarisation
+// (inputs E_p[k] and E_p[k] W_2048^-k share the transform's twiddles), the polarisations follow one another.
+// Re z then leaves the transform as the (even, odd) pair an 8-byte store wants: no parking of samples, no register
+// shuffles to pair them up; |z_theta|^2 of both samples waits in tensor memory for |z_phi|^2.
+template <class G>
+__device__ __forceinline__ void build_inverse_input_eo(R (&Zr)[32], R (&Zi)[32], const float2 *TS, int lane, uint32_t tstash_p)
+{
+    // tstash_p = stash + polarisation: columns 4 r + p (Re E_p) and 4 r + 2 + p (Im E_p) of band row r
+    uint32_t er[G::kBandRows], ei[G::kBandRows];
+    static_for<0, G::kBandRows>([&](auto rc) {
+        constexpr int r = decltype(rc)::value;
+        er[r] = tmem_ld32(tstash_p + 4 * r);
+        ei[r] = tmem_ld32(tstash_p + 4 * r + 2);
+    });
+    tmem_wait_ld();
+    static_for<0, 32>([&](auto kc) {
+        constexpr int k2 = decltype(kc)::value;
+        if constexpr (k2 < G::kLo || k2 > G::kHi) { Zr[brev5(k2)] = L::zero(); Zi[brev5(k2)] = L::zero(); }
+        else {
+            constexpr int r = k2 - G::kLo;
+            tmem_ld_dep32(er[r], ei[r]);
+            const float2 w = TS[lane + 32 * k2];
+            const float sr = __uint_as_float(er[r]), si = __uint_as_float(ei[r]);
+            // odd samples: (sr + i si)(wr - i wi)
+            const float orr = fmaf(si, w.y, sr * w.x), oi = fmaf(-sr, w.y, si * w.x);
+            Zr[brev5(k2)] = L::pack(sr, orr);
+            Zi[brev5(k2)] = L::pack(si, oi);
+        }
+    });
+}
+
+// theta pass: store Re z_theta as (even, odd) pairs, park |z_theta|^2 of both samples
+template <bool HAS_EF>
+__device__ __forceinline__ void emit_theta(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef)
+{
+    static_for<0, 32>([&](auto bc) {
+        constexpr int b = decltype(bc)::value;
+        if (HAS_EF) st_global_b64(ef + 2 * (lane + 32 * b), zr[b]);
+        R q = L::mul(zr[b], zr[b]);
+        q = L::fma(zi[b], zi[b], q);
+        tmem_st64(tpark + 2 * b, q.v);
+    });
+}
+
+// phi pass: store Re z_phi, env^2 = parked |z_theta|^2 + |z_phi|^2 for the even and the odd sample of every row,
+// running (max, lowest row) per parity
+template <bool HAS_EF>
+__device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef,
+                                         float &best0, int &b0, float &best1, int &b1)
+{
+    tmem_wait_st();
+    static_for<0, 4>([&](auto cc) {
+        constexpr int c = decltype(cc)::value;
+        unsigned long long ev[8];
+        static_for<0, 8>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            ev[j] = tmem_ld64(tpark + 2 * (8 * c + j));
+        });
+        tmem_wait_ld();
+        static_for<0, 4>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            tmem_ld_dep(ev[2 * j], ev[2 * j + 1]);
+        });
+        static_for<0, 8>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            constexpr int b = 8 * c + j;
+            if (HAS_EF) st_global_b64(ef + 2 * kM + 2 * (lane + 32 * b), zr[b]);
+            R q; q.v = ev[j];
+            q = L::fma(zr[b], zr[b], q);
+            q = L::fma(zi[b], zi[b], q);
+            float e0, e1;
+            L::unpack(q, e0, e1);
+            if (e0 > best0) { best0 = e0; b0 = b; }
+            if (e1 > best1) { best1 = e1; b1 = b; }
+        });
+    });
+}
+
 // Per-instantiation geometry: shared memory per warp, tensor-memory columns per warp, warps per CTA.
 template <int K2LO, int K2HI>
 struct W32Geom {
