@@ -331,11 +331,12 @@ unfold_w32_kernel(W32Params p)
                 const int n1 = 2 * (lane + 32 * b1) + 1;
                 if (best1 > best || (best1 == best && n1 < bi)) { best = best1; bi = n1; }
             }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+            // env^2 >= 0, so the float order is the order of the bit patterns: two warp-wide integer reductions
+            // (REDUX) instead of five shuffle stages: the maximum, then the lowest index among the lanes that hold it
+            {
+                const unsigned bmax = __reduce_max_sync(0xffffffffu, __float_as_uint(best));
+                bi = (int)__reduce_min_sync(0xffffffffu, __float_as_uint(best) == bmax ? (unsigned)bi : 0xffffffffu);
+                best = __uint_as_float(bmax);
             }
             if (lane == 0) { p.amp[u] = sqrtf(best); p.idx[u] = bi; }
         }
