@@ -84,7 +84,11 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
 //                 band are never written or used                                       (team kernel)
 //   MINV_Q32    : per direction 64 float4 planes [q = k & 31][A | B as in MINV_PACKED][C], column
 //                 (k >> 5) - (k_lo >> 5), C = (k_hi >> 5) - (k_lo >> 5) + 1              (long-trace kernel)
-enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3 };
+//   MINV_PACKED_PAD : MINV_PACKED with 32 zero entries before and after each plane (planes of K + 64 entries, bin j at
+//                 index j + 32): a warp kernel whose edge rows reach up to 31 bins beyond the band multiplies by zero
+//                 there instead of clamping the index and selecting                       (batch warp kernel)
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3, MINV_PACKED_PAD = 4 };
+constexpr int kMinvPad = 32;
 // complex elements per direction in the MINV_Q4 layout (<= 4 K + 32)
 __host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,

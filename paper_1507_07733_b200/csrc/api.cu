@@ -264,7 +264,7 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
     WsLayout w{};
     const size_t cb = cplx_bytes(dtype);
     size_t o = 0;
-    size_t per_dir = (size_t)K * 4 + 32;                                  // + 32: MINV_Q4 plane padding
+    size_t per_dir = (size_t)K * 4 + 8 * kMinvPad;                        // MINV_PACKED_PAD planes (covers MINV_Q4's + 32 too)
     const size_t q32 = (size_t)128 * ((k_hi >> 5) - (k_lo >> 5) + 1);     // MINV_Q32 planes
     if (q32 > per_dir) per_dir = q32;
     w.off_minv = o; o = align_up(o + (size_t)n_patterns * n_dirs * per_dir * cb);   // one slab of n_dirs matrices per table
@@ -502,10 +502,11 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     const bool warp_path = fast && w32_supported(dtype, pl->dev);
     const bool team_path = fast && !ext.input_i16 && t4k_f64_supported(dtype, pl->dev);
     const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
-    const int layout = warp_path ? MINV_PACKED : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS));
+    const int layout = warp_path ? MINV_PACKED_PAD : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS));
     // complex elements of one event's matrices in this layout; the tables' slabs follow one another
     const size_t per_event = layout == MINV_Q4 ? minv_q4_stride(pl->dev.k_lo, pl->dev.k_hi)
-                             : (layout == MINV_Q32 ? (size_t)128 * ((pl->dev.k_hi >> 5) - (pl->dev.k_lo >> 5) + 1) : (size_t)pl->dev.K * 4);
+                             : (layout == MINV_Q32 ? (size_t)128 * ((pl->dev.k_hi >> 5) - (pl->dev.k_lo >> 5) + 1)
+                                                   : (layout == MINV_PACKED_PAD ? (size_t)(pl->dev.K + 2 * kMinvPad) * 4 : (size_t)pl->dev.K * 4));
     UnfoldExt x;
     x.pattern_id = ext.pattern_id;
     x.minv_pattern_stride = (size_t)n_events * per_event;

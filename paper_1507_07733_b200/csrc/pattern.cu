@@ -168,11 +168,25 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
             cx<T> *b = a + (size_t)C * 2;
             a[0].re = mt0.re; a[0].im = mp0.re; a[1].re = mt0.im; a[1].im = mp0.im;
             b[0].re = mt1.re; b[0].im = mp1.re; b[1].re = mt1.im; b[1].im = mp1.im;
+        } else if (layout == MINV_PACKED_PAD) {
+            const int KP = K + 2 * kMinvPad;
+            cx<T> *a = minv + (size_t)d * KP * 4 + (size_t)(j + kMinvPad) * 2, *b = a + (size_t)KP * 2;
+            a[0].re = mt0.re; a[0].im = mp0.re; a[1].re = mt0.im; a[1].im = mp0.im;
+            b[0].re = mt1.re; b[0].im = mp1.re; b[1].re = mt1.im; b[1].im = mp1.im;
         } else { // MINV_PACKED: two planes per direction, (theta, phi) side by side so a packed
                  // f32x2 load yields both: A[j] = {t0.re, p0.re, t0.im, p0.im}, B[j] = {t1.re, p1.re, t1.im, p1.im}
             cx<T> *a = minv + (size_t)d * K * 4 + (size_t)j * 2, *b = a + (size_t)K * 2;
             a[0].re = mt0.re; a[0].im = mp0.re; a[1].re = mt0.im; a[1].im = mp0.im;
             b[0].re = mt1.re; b[0].im = mp1.re; b[1].re = mt1.im; b[1].im = mp1.im;
+        }
+    }
+    if (layout == MINV_PACKED_PAD) { // the zero pads before and after both planes
+        const int KP = K + 2 * kMinvPad;
+        const cx<T> z = {(T)0, (T)0};
+        for (int j = threadIdx.x; j < kMinvPad; j += blockDim.x) {
+            cx<T> *a0 = minv + (size_t)d * KP * 4 + (size_t)j * 2, *a1 = a0 + (size_t)(K + kMinvPad) * 2;
+            a0[0] = z; a0[1] = z; a1[0] = z; a1[1] = z;
+            a0[(size_t)KP * 2] = z; a0[(size_t)KP * 2 + 1] = z; a1[(size_t)KP * 2] = z; a1[(size_t)KP * 2 + 1] = z;
         }
     }
 }

@@ -62,7 +62,7 @@ struct W32Params {
     float *efield;
     float *amp;
     int32_t *idx;
-    const float4 *minv;   // [n_events] { A[K], B[K] } float4, see MINV_PACKED
+    const float4 *minv;   // [n_events] { A[K + 64], B[K + 64] } float4, see MINV_PACKED_PAD
     float4 *spectra;      // [n_units][band rows][32] {2V0.re, 2V0.im, 2V1.re, 2V1.im}: written (SPEC 1) or read (SPEC 2)
     const float2 *tw1024; // W_1024^m
     const float2 *twN;    // W_2048^m
@@ -90,9 +90,12 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
     for (int r = 0; r < G::kBandRows; ++r, own += 32, par -= 32, k += 32) {
         // branch-free: rows at the band edges read a clamped Minv entry and select zero afterwards, so the
         // loads of neighbouring rows are independent and the unrolled iterations overlap their latencies
-        const bool inband = k >= k_lo && k <= k_hi;
+        // rows of a band-specific instantiation reach at most 31 bins beyond the band: Minv is zero-padded there
+        // (MINV_PACKED_PAD), so E = 0 comes out of the arithmetic; the any-band instantiation clamps and selects
+        constexpr bool kAnyBand = G::kLo == 0 && G::kHi == 31;
+        const bool inband = !kAnyBand || (k >= k_lo && k <= k_hi);
         int j = k - k_lo;
-        j = j < 0 ? 0 : (j > k_hi - k_lo ? k_hi - k_lo : j);
+        if (kAnyBand) j = j < 0 ? 0 : (j > k_hi - k_lo ? k_hi - k_lo : j);
         // (lane 0 of row 0 would look for its mirror in row 32: k = 0 is never in band, keep the read inside the buffer)
         const int pc = (G::kLo == 0 && par > G::kPubRows * 32 - 1) ? G::kPubRows * 32 - 1 : par;
         const R ar = QA[own], ai = QB[own], pr = QA[pc], pi = QB[pc];
@@ -109,7 +112,7 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
         float v0i = fmaf(w.x, f0i1, f0i0); v0i = fmaf(w.y, f0r1, v0i);
         float v1r = fmaf(w.x, f1r1, f1r0); v1r = fmaf(-w.y, f1i1, v1r);
         float v1i = fmaf(w.x, f1i1, f1i0); v1i = fmaf(w.y, f1r1, v1i);
-        if (!inband) { v0r = 0.f; v0i = 0.f; v1r = 0.f; v1i = 0.f; }
+        if (kAnyBand && !inband) { v0r = 0.f; v0i = 0.f; v1r = 0.f; v1i = 0.f; }
         const R Ma = L::pack(m0.x, m0.y), Mb = L::pack(m0.z, m0.w), Mc = L::pack(m1.x, m1.y), Md = L::pack(m1.z, m1.w);
         R er = L::mul(Ma, L::bc(v0r)); er = L::fma(Mb, L::bc(-v0i), er);
         er = L::fma(Mc, L::bc(v1r), er); er = L::fma(Md, L::bc(-v1i), er);
@@ -166,7 +169,8 @@ unfold_w32_kernel(W32Params p)
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + kTabBytes);     // [2] Minv slot filled
     int *done = reinterpret_cast<int *>(smem + kTabBytes + 16);          // [2] warps finished with the slot
     uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabBytes + 32);
-    const uint32_t minv_bytes = (uint32_t)p.K * 32u;
+    const int KP = p.K + 2 * kMinvPad;                          // entries per padded Minv plane
+    const uint32_t minv_bytes = (uint32_t)KP * 32u;
     const uint32_t slot_bytes = MINV_SMEM ? ((minv_bytes + 127u) & ~127u) : 0u;
     unsigned char *mslot = smem + kTabBytes + kCtlBytes;
     // warp index through a shuffle: provably warp-uniform, so everything derived from it is too
@@ -190,7 +194,7 @@ unfold_w32_kernel(W32Params p)
         done[0] = 0; done[1] = 0;
         for (int s = 0; s < 2 && e0 + s <= e1; ++s) {
             mbar_expect_tx(&full[s], minv_bytes);
-            tma_bulk_g2s(mslot + (size_t)s * slot_bytes, p.minv + (size_t)(e0 + s) * p.K * 2, minv_bytes, &full[s]);
+            tma_bulk_g2s(mslot + (size_t)s * slot_bytes, p.minv + (size_t)(e0 + s) * KP * 2, minv_bytes, &full[s]);
         }
     }
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
@@ -213,8 +217,7 @@ unfold_w32_kernel(W32Params p)
         const long hi = u1 < (e + 1) * S ? u1 : (e + 1) * S;
         const long first = lo + (((long)warp - (lo - u0)) % kWarps + kWarps) % kWarps;
         const float4 *MA = MINV_SMEM ? reinterpret_cast<const float4 *>(mslot + (size_t)slot * slot_bytes)
-                                     : p.minv + (size_t)e * p.K * 2;
-        const float4 *MB = MA + p.K;
+                                     : p.minv + (size_t)e * KP * 2;
         bool minv_ready = !MINV_SMEM;
 
 #pragma unroll 1
@@ -222,8 +225,8 @@ unfold_w32_kernel(W32Params p)
             const float *v = static_cast<const float *>(p.traces) + (size_t)u * 4 * kM;
             const int16_t *v16 = static_cast<const int16_t *>(p.traces) + (size_t)u * 4 * kM;
             // several tables resident: this station's antenna type selects the Minv slab (read through L1/L2)
-            const float4 *MAu = (MINV_SMEM || p.pattern_id == nullptr) ? MA : MA + (size_t)p.pattern_id[u - e * S] * p.minv_pattern_stride;
-            const float4 *MBu = MAu + p.K;
+            const float4 *MAu = ((MINV_SMEM || p.pattern_id == nullptr) ? MA : MA + (size_t)p.pattern_id[u - e * S] * p.minv_pattern_stride) + kMinvPad;
+            const float4 *MBu = MAu + KP;
             float *ef = HAS_EF ? p.efield + (size_t)u * 4 * kM : nullptr;
             float4 *sp = SPEC != 0 ? p.spectra + (size_t)u * G::kBandRows * 32 + lane : nullptr;
             if (AERA_PREFETCH_DIST > 0 && lane == 0 && u + AERA_PREFETCH_DIST * kWarps < u1) {
@@ -355,7 +358,7 @@ unfold_w32_kernel(W32Params p)
                     if (e + 2 <= e1) {
                         fence_proxy_async_smem();
                         mbar_expect_tx(&full[slot], minv_bytes);
-                        tma_bulk_g2s(mslot + (size_t)slot * slot_bytes, p.minv + (size_t)(e + 2) * p.K * 2, minv_bytes, &full[slot]);
+                        tma_bulk_g2s(mslot + (size_t)slot * slot_bytes, p.minv + (size_t)(e + 2) * KP * 2, minv_bytes, &full[slot]);
                     }
                 }
             }
@@ -370,7 +373,7 @@ template <int K2LO, int K2HI, bool MINV_SMEM>
 size_t w32_smem_bytes(int K)
 {
     using G = W32Geom<K2LO, K2HI>;
-    const size_t slot = MINV_SMEM ? (((size_t)K * 32 + 127) & ~(size_t)127) : 0;
+    const size_t slot = MINV_SMEM ? (((size_t)(K + 2 * kMinvPad) * 32 + 127) & ~(size_t)127) : 0;
     return (size_t)kTabBytes + kCtlBytes + 2 * slot + (size_t)G::kWarps * G::kWarpBytes;
 }
 
