@@ -3,7 +3,7 @@
 // for the scan mode") and of the FP32 / FP64 co-limiter figures in DESIGN.md section 5.
 //
 // Each kernel is a register-only chain of independent fused multiply-adds, 8 accumulators per thread,
-// unrolled 8x, one CTA per SM x `ctas_per_sm`, so the only limiter is the issue rate of the pipe:
+// unrolled 32x, one CTA per SM x `ctas_per_sm`, so the only limiter is the issue rate of the pipe:
 //   kind 0  fma.rn.f32x2 (SASS FFMA2): two fp32 FMAs per lane per instruction (the warp kernels' form)
 //   kind 1  fma.rn.f32   (SASS FFMA)
 //   kind 2  fma.rn.f64   (SASS DFMA)
@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(1024, 1) alu_peak_kernel(double *out, int iter
 #pragma unroll 1
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
-            for (int u = 0; u < 8; ++u)
+            for (int u = 0; u < 32; ++u)
 #pragma unroll
                 for (int i = 0; i < 8; ++i) x[i] = LaneF32x2::fma(x[i], pa, pb);
         }
@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(1024, 1) alu_peak_kernel(double *out, int iter
 #pragma unroll 1
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
-            for (int u = 0; u < 8; ++u)
+            for (int u = 0; u < 32; ++u)
 #pragma unroll
                 for (int i = 0; i < 8; ++i) x[i] = fmaf(x[i], a, b);
         }
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(1024, 1) alu_peak_kernel(double *out, int iter
 #pragma unroll 1
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
-            for (int u = 0; u < 8; ++u)
+            for (int u = 0; u < 32; ++u)
 #pragma unroll
                 for (int i = 0; i < 8; ++i) x[i] = fma(x[i], da, db);
         }
@@ -78,7 +78,7 @@ cudaError_t run_kind(int sms, int warps, int iters, double *d_out, double *lane_
         e = cudaEventSynchronize(e1);
         float ms = 0.f;
         if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-        const double fmas = (double)sms * warps * 32 * (double)iters * 64.0 * (KIND == 0 ? 2.0 : 1.0);
+        const double fmas = (double)sms * warps * 32 * (double)iters * 256.0 * (KIND == 0 ? 2.0 : 1.0);
         if (e == cudaSuccess && ms > 0.f && fmas / (ms * 1e-3) > best) best = fmas / (ms * 1e-3);
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
@@ -99,7 +99,7 @@ cudaError_t measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s,
     double *d_out = nullptr;
     e = cudaMalloc((void **)&d_out, (size_t)sms * 1024 * sizeof(double));
     if (e != cudaSuccess) return e;
-    const int iters = 4000;
+    const int iters = 1000;
     if (kind == 0) e = run_kind<0>(sms, warps_per_sm, iters, d_out, lane_fma_per_s);
     else if (kind == 1) e = run_kind<1>(sms, warps_per_sm, iters, d_out, lane_fma_per_s);
     else e = run_kind<2>(sms, warps_per_sm, iters, d_out, lane_fma_per_s);

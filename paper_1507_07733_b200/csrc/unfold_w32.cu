@@ -208,6 +208,7 @@ unfold_w32_kernel(W32Params p)
     const uint32_t tbase = *tmem_base;
     const uint32_t tstash = tmem_addr(tbase, warp, (warp >> 2) * G::kColStride);
     const uint32_t tpark = tstash + G::kParkCol;
+    const unsigned long long pol_first = l2_policy_evict_first();
 
 #pragma unroll 1
     for (long e = e0; e <= e1; ++e) {
@@ -319,14 +320,14 @@ unfold_w32_kernel(W32Params p)
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
                 } else
-                    emit_theta<HAS_EF>(B, A, lane, tpark, ef);
+                    emit_theta<HAS_EF>(B, A, lane, tpark, ef, pol_first);
                 // ---- a5 (one copy of the code for both polarisations; the registers are dead at this join):
                 // (z[2m], z[2m+1]) = IFFT_1024 of (E_p, E_p W_2048^-k), p = theta after t = 0, phi after t = 1;
                 // inverse roles, A = Im, B = Re
                 build_inverse_input_eo<G>(B, A, TS, lane, tstash + (uint32_t)t);
                 ++t;
             }
-            emit_phi<HAS_EF>(B, A, lane, tpark, ef, best0, b0, best1, b1);
+            emit_phi<HAS_EF>(B, A, lane, tpark, ef, pol_first, best0, b0, best1, b1);
 
             // ---- a6: lane result (lowest index on ties), then warp argmax with the same rule
             float best = best0; int bi = 2 * (lane + 32 * b0);

@@ -82,9 +82,28 @@ __device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const floa
 #ifndef AERA_W32_ABLATE
 #define AERA_W32_ABLATE 0   // timing experiments only, see unfold_w32.cu
 #endif
+#ifndef AERA_W32_ST_POLICY
+#define AERA_W32_ST_POLICY 1   // 1: E-field stores carry an L2 evict_first hint (the written lines do not push the L2-prefetched traces out)
+#endif
+__device__ __forceinline__ unsigned long long l2_policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// streamed output: the line leaves the L2 first
+__device__ __forceinline__ void st_global_b64_stream(void *p, R v, unsigned long long pol)
+{
+#if AERA_W32_ST_POLICY == 1
+    asm volatile("st.global.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(p), "l"(v.v), "l"(pol) : "memory");
+#else
+    asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
+#endif
+}
 __device__ __forceinline__ void st_global_b64(void *p, R v)
 {
     if ((AERA_W32_ABLATE & 4) && v.v != 0x123456789abcdefull) return;
+
     asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
 }
 
@@ -187,11 +206,11 @@ __device__ __forceinline__ void build_inverse_input_eo(R (&Zr)[32], R (&Zi)[32],
 
 // theta pass: store Re z_theta as (even, odd) pairs, park |z_theta|^2 of both samples
 template <bool HAS_EF>
-__device__ __forceinline__ void emit_theta(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef)
+__device__ __forceinline__ void emit_theta(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef, unsigned long long pol)
 {
     static_for<0, 32>([&](auto bc) {
         constexpr int b = decltype(bc)::value;
-        if (HAS_EF) st_global_b64(ef + 2 * (lane + 32 * b), zr[b]);
+        if (HAS_EF && !(AERA_W32_ABLATE & 4)) st_global_b64_stream(ef + 2 * (lane + 32 * b), zr[b], pol);
         R q = L::mul(zr[b], zr[b]);
         q = L::fma(zi[b], zi[b], q);
         tmem_st64(tpark + 2 * b, q.v);
@@ -201,7 +220,7 @@ __device__ __forceinline__ void emit_theta(const R (&zr)[32], const R (&zi)[32],
 // phi pass: store Re z_phi, env^2 = parked |z_theta|^2 + |z_phi|^2 for the even and the odd sample of every row,
 // running (max, lowest row) per parity
 template <bool HAS_EF>
-__device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef,
+__device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], int lane, uint32_t tpark, float *ef, unsigned long long pol,
                                          float &best0, int &b0, float &best1, int &b1)
 {
     tmem_wait_st();
@@ -220,7 +239,7 @@ __device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], i
         static_for<0, 8>([&](auto jc) {
             constexpr int j = decltype(jc)::value;
             constexpr int b = 8 * c + j;
-            if (HAS_EF) st_global_b64(ef + 2 * kM + 2 * (lane + 32 * b), zr[b]);
+            if (HAS_EF && !(AERA_W32_ABLATE & 4)) st_global_b64_stream(ef + 2 * kM + 2 * (lane + 32 * b), zr[b], pol);
             R q; q.v = ev[j];
             q = L::fma(zr[b], zr[b], q);
             q = L::fma(zi[b], zi[b], q);
