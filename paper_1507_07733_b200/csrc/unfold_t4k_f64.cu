@@ -72,6 +72,17 @@ __device__ __forceinline__ double ld_stream_f64(const double *p)
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 }
+// streamed output with an L2 evict_first policy: the written lines leave the L2 before the L2-prefetched traces do
+__device__ __forceinline__ unsigned long long t4k_policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void st_stream_f64(double *p, double v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
 __device__ __forceinline__ double2 ld_nc_d2(const double2 *p)
 {
     double2 r;
@@ -177,6 +188,7 @@ unfold_t4k_f64_kernel(T4kParams p)
     const uint32_t tenv = tmem_addr(*tmem_base, warp, team * 128); // |z_theta|^2: 2 columns per sample, 64 columns
     const uint32_t tephi = tenv + 64;                               // E_phi: 4 columns per band row
 
+    const unsigned long long pol_first = t4k_policy_evict_first();
     const long u0 = p.n_units * (long)blockIdx.x / (long)gridDim.x;
     const long u1 = p.n_units * ((long)blockIdx.x + 1) / (long)gridDim.x;
     constexpr int N = 4096;
@@ -381,7 +393,7 @@ unfold_t4k_f64_kernel(T4kParams p)
             if (pol == 0) {
                 static_for<0, 32>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    if (HAS_EF) ef[nbase + 32 * (i & 7) + 1024 * (i >> 3)] = P[i];
+                    if (HAS_EF) st_stream_f64(ef + nbase + 32 * (i & 7) + 1024 * (i >> 3), P[i], pol_first);
                     double e2 = P[i] * P[i]; e2 = fma(Q[i], Q[i], e2);
                     tmem_st64(tenv + 2 * i, (unsigned long long)__double_as_longlong(e2));
                 });
@@ -403,7 +415,7 @@ unfold_t4k_f64_kernel(T4kParams p)
                         constexpr int j = decltype(jc)::value;
                         constexpr int i = 8 * c + j;
                         const int n = nbase + 32 * (i & 7) + 1024 * (i >> 3);
-                        if (HAS_EF) ef[N + n] = P[i];
+                        if (HAS_EF) st_stream_f64(ef + N + n, P[i], pol_first);
                         double e2 = fma(P[i], P[i], __longlong_as_double((long long)ev[j]));
                         e2 = fma(Q[i], Q[i], e2);
                         if (e2 > best) { best = e2; bn = n; }

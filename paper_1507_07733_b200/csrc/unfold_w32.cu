@@ -38,6 +38,9 @@
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
 #include "w32_common.cuh"
 
+#ifndef AERA_W32_LD_POLICY
+#define AERA_W32_LD_POLICY 0
+#endif
 #ifndef AERA_W32_ABLATE
 #define AERA_W32_ABLATE 0   // timing experiments only (wrong results), bit mask: 1 no fft32, 2 no transposes, 4 no global loads/stores, 8 no pass twiddles, 16 no separation+solve, 32 no envelope/argmax
 #endif
@@ -248,8 +251,13 @@ unfold_w32_kernel(W32Params p)
                         B[brev5(j)] = L::pack((float)(short)(b & 0xffff), (float)(b >> 16));
                         return;
                     }
+#if AERA_W32_LD_POLICY
+                    A[brev5(j)] = ld_stream_b64_pol(v + 2 * (lane + 32 * j), pol_first);            // (v0[2m], v0[2m+1])
+                    B[brev5(j)] = ld_stream_b64_pol(v + 2 * kM + 2 * (lane + 32 * j), pol_first);   // (v1[2m], v1[2m+1])
+#else
                     A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
                     B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
+#endif
                 });
             } else {
                 // ---- the forward spectrum of this station was stored by an earlier call: a4 straight away

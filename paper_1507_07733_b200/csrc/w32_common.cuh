@@ -24,6 +24,12 @@ __device__ __forceinline__ R ld_stream_b64(const void *p)
     asm volatile("ld.global.nc.L1::no_allocate.b64 %0, [%1];" : "=l"(r.v) : "l"(p));
     return r;
 }
+__device__ __forceinline__ R ld_stream_b64_pol(const void *p, unsigned long long pol)
+{
+    R r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(r.v) : "l"(p), "l"(pol));
+    return r;
+}
 __device__ __forceinline__ int ld_stream_b32(const void *p)
 {
     int r;
