@@ -224,17 +224,14 @@ unfold_long_f32_kernel(LongParams p)
     R *YA = reinterpret_cast<R *>(sc), *YB = YA + 32 * 1024;
     R *EA = reinterpret_cast<R *>(sc + kYBytes), *EB = EA + 32 * p.C;
     R *H0 = EB + 32 * p.C;                                              // [pol 2][t 16][mm 1024] parked (s = 0, 1) pairs
+    R *U0 = H0 + 2 * 16 * 1024;                                         // U[2][16][1024] two 8-byte planes
     const int C = p.C, c_lo = p.k_lo >> 5;
     const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
 
-#pragma unroll 1
-    for (long u = cluster_id; u < p.n_units; u += n_clusters) {
-        const float *v0 = p.traces + (size_t)u * 2 * kLN, *v1 = v0 + kLN;
-        float *ef = HAS_EF ? p.efield + (size_t)u * 2 * kLN : nullptr;
-        const long ev = u / p.n_stations;
-        const float4 *Mev = p.minv + (size_t)ev * 64 * C + (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
-
-        // ---------------- phase 1: loads + 32-point transform over j' + twiddle -> Y
+    // ---------------- phase 1 of station uu: loads + 32-point transform over j' + twiddle -> Y. It depends on nothing but
+    // the free Y buffer, so it runs in the same round as phase 4 of the previous station (no barrier between them).
+    auto phase1 = [&](long uu) {
+        const float *v0 = p.traces + (size_t)uu * 2 * kLN, *v1 = v0 + kLN;
 #pragma unroll 1
         for (int mb = gw; mb < 32; mb += kLTeam) {
             const int mm = lane + 32 * mb;
@@ -259,7 +256,15 @@ unfold_long_f32_kernel(LongParams p)
                 st_sc(YB + q * 1024 + mm, B[q], pol_last);
             });
         }
-        cluster_sync_all();
+    };
+    if (cluster_id < p.n_units) phase1(cluster_id);
+    cluster_sync_all();
+
+#pragma unroll 1
+    for (long u = cluster_id; u < p.n_units; u += n_clusters) {
+        float *ef = HAS_EF ? p.efield + (size_t)u * 2 * kLN : nullptr;
+        const long ev = u / p.n_stations;
+        const float4 *Mev = p.minv + (size_t)ev * 64 * C + (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
 
         // ---------------- phase 2: 1024-point transform per q, separation with the pair partner, fold, a4 -> E
 #pragma unroll 1
@@ -317,7 +322,8 @@ unfold_long_f32_kernel(LongParams p)
         }
         cluster_sync_all();
 
-        R *UA = YA, *UB = YB;                           // U[sl][q'][mm] reuses Y (index (16 sl + q') * 1024 + mm)
+        R *UA = U0, *UB = U0 + 32 * 1024;               // U[sl][q'][mm] (index (16 sl + q') * 1024 + mm), its own buffer:
+                                                        // Y is being refilled by the next station's phase 1 meanwhile
         float best = -1.0f; int bn = 0;
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
@@ -407,6 +413,8 @@ unfold_long_f32_kernel(LongParams p)
             }
             if (h == 0) cluster_sync_all();                          // U is rewritten by the next pair's phase 3
         }
+        // ---------------- phase 1 of the next station, in the same round as this station's last phase 4
+        if (u + n_clusters < p.n_units) phase1(u + n_clusters);
         // ---------------- a6: lane -> warp -> CTA argmax (lowest index on ties: key = value bits, ~index)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -421,7 +429,7 @@ unfold_long_f32_kernel(LongParams p)
             asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(gpeak + crank), "l"(*peak) : "memory");
             *peak = 0ull;
         }
-        cluster_sync_all();                                          // also: next station's phase 1 may overwrite Y / U
+        cluster_sync_all();                                          // also: Y of the next station is complete, U is free
         if (crank == 0 && threadIdx.x == 0) {
             unsigned long long key = 0ull;
 #pragma unroll
@@ -448,7 +456,7 @@ bool long_f32_supported(int dtype, const PlanDev &p)
 static size_t long_stride(const PlanDev &p)
 {
     const size_t C = (size_t)((p.k_hi >> 5) - (p.k_lo >> 5) + 1);
-    return (kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | per-CTA peaks
+    return (2 * kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | U | per-CTA peaks
 }
 size_t long_f32_scratch_bytes(const PlanDev &p) { return long_max_clusters() * long_stride(p); }
 
