@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -730,8 +731,9 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
     const size_t rb = real_bytes(dtype);
     const size_t unit_bytes = (size_t)2 * n_samples * rb;
     const size_t event_bytes = unit_bytes * n_stations;
-    // chunk: ~64 MB of traces per stage, at least one event
-    long chunk_events = (long)((size_t)(64u << 20) / event_bytes);
+    // chunk: ~64 MB of traces per stage (AERA_HOST_CHUNK_MB overrides, tuning only), at least one event
+    static const size_t chunk_mb = [] { const char *e = getenv("AERA_HOST_CHUNK_MB"); const int v = e ? atoi(e) : 64; return (size_t)(v < 1 ? 1 : (v > 1024 ? 1024 : v)); }();
+    long chunk_events = (long)((chunk_mb << 20) / event_bytes);
     if (chunk_events < 1) chunk_events = 1;
     if (chunk_events > n_events) chunk_events = n_events;
 
