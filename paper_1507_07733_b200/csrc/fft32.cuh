@@ -132,4 +132,36 @@ __device__ __forceinline__ void fft32(typename L::R (&re)[32], typename L::R (&i
     });
 }
 
+// The same transform when only the input ELEMENTS NZLO..NZHI are non-zero (the first pass of an inverse transform whose
+// spectrum is confined to the band rows): in stage 0, which pairs element e with e + 16, a butterfly with one zero
+// input is a copy (b = 0) or a copy and a negation (a = 0; ptxas folds the negation into the consumers' operand
+// modifiers), with two zero inputs nothing. The zero elements are never read, so the caller need not store them.
+// (From stage 1 on every value is non-zero for the bands of interest and the stages are the plain ones.)
+template <class L, int NZLO, int NZHI>
+__device__ __forceinline__ void fft32_pruned(typename L::R (&re)[32], typename L::R (&im)[32])
+{
+    static_for<0, 16>([&](auto bc) {
+        constexpr int b = decltype(bc)::value;
+        constexpr int i0 = 2 * b, i1 = i0 + 1;
+        constexpr int e0 = brev5(i0), e1 = brev5(i1);        // element indices: e1 = e0 + 16
+        constexpr bool za = e0 < NZLO || e0 > NZHI, zb = e1 < NZLO || e1 > NZHI;
+        if constexpr (za && zb) { re[i0] = L::zero(); im[i0] = L::zero(); re[i1] = L::zero(); im[i1] = L::zero(); }
+        else if constexpr (zb) { re[i1] = re[i0]; im[i1] = im[i0]; }
+        else if constexpr (za) { re[i0] = re[i1]; im[i0] = im[i1]; re[i1] = L::neg(re[i1]); im[i1] = L::neg(im[i1]); }
+        else butterfly<L, 0>(re[i0], im[i0], re[i1], im[i1]);
+    });
+    static_for<1, 5>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        constexpr int half = 1 << s;
+        static_for<0, 16>([&](auto bc) {
+            constexpr int b = decltype(bc)::value;
+            constexpr int j = b & (half - 1);
+            constexpr int i0 = ((b - j) << 1) + j;
+            constexpr int i1 = i0 + half;
+            constexpr int idx = j * (16 >> s);
+            butterfly<L, idx>(re[i0], im[i0], re[i1], im[i1]);
+        });
+    });
+}
+
 } // namespace aera

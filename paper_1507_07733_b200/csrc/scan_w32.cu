@@ -236,28 +236,27 @@ scan_inv_w32_kernel(ScanParams p)
             }
             // ---- a5/a6: even samples, then odd samples, through ONE copy of the FFT code
             float best0 = -1.0f, best1 = -1.0f; int b0 = 0, b1 = 0;
+            // bottom-tested loop with an opaque counter: ONE copy of the two-pass transform for the even (tpass = 1) and
+            // the odd (tpass = 2) samples (a loop with the exit in the middle is rotated, which duplicates the transforms)
             int tpass = 1;
 #pragma unroll 1
-            for (;;) {
-                int second = 0;
-                asm volatile("" : "+r"(second));
-#pragma unroll 1
-                for (;;) {
-                    fft32<L>(A, B);
-                    if (second) break;
-                    pass_twiddle(A, B, T, lane);
-                    transpose_plane(A, X, lane);
-                    transpose_plane(B, X, lane);
-                    second = 1;
-                    asm volatile("" : "+r"(second));
-                }
-                if (tpass == 2) break;
-                emit_even<false>(B, A, 0u, best0, b0);
-                tmem_wait_st();
-                build_inverse_input<G, true>(B, A, TS, lane, tstash);
+            do {
+                // every transform of this kernel is an inverse one whose input is confined to the band rows: the first
+                // pass runs the pruned 32-point transform (13 of its 16 first-stage butterflies are copies at configs[2])
+                fft32_pruned<L, G::kLo, G::kHi>(A, B);
+                pass_twiddle(A, B, T, lane);
+                transpose_plane(A, X, lane);
+                transpose_plane(B, X, lane);
+                fft32<L>(A, B);
+                asm volatile("" : "+r"(tpass));
+                if (tpass == 1) {
+                    emit_even<false>(B, A, 0u, best0, b0);
+                    tmem_wait_st();
+                    build_inverse_input<G, true>(B, A, TS, lane, tstash);
+                } else
+                    emit_odd<false>(B, A, lane, 0u, nullptr, best1, b1);
                 ++tpass;
-            }
-            emit_odd<false>(B, A, lane, 0u, nullptr, best1, b1);
+            } while (tpass <= 2);
             float best = best0; int bi = 2 * (lane + 32 * b0);
             {
                 const int n1 = 2 * (lane + 32 * b1) + 1;
