@@ -27,33 +27,59 @@ __device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b)
     return r;
 }
 
-// In-place radix-2 decimation-in-time FFT of `nbuf` buffers of N points whose inputs are already
-// in bit-reversed order. tw[m] = exp(-2 pi i m / N), m < N/2; inverse uses the conjugate.
+// In-place decimation-in-time FFT of NBUF buffers of N points whose inputs are already in bit-reversed order.
+// tw[m] = exp(-2 pi i m / N), m < N/2; inverse uses the conjugate. Three radix-2 stages are fused into one
+// radix-8 pass per trip through shared memory (each thread holds the 8 points i0 + t 2^s, t = 0..7, of a group in
+// registers), preceded by one radix-2 or radix-4 pass when log2 N is not a multiple of 3: a third of the
+// barriers and of the shared-memory traffic of the stage-by-stage form.
+template <typename T, bool INVERSE>
+__device__ __forceinline__ void bfly(cx<T> &a, cx<T> &b, cx<T> w)
+{
+    if (INVERSE) w.im = -w.im;
+    const cx<T> t = cmul(w, b);
+    b.re = a.re - t.re; b.im = a.im - t.im;
+    a.re = a.re + t.re; a.im = a.im + t.im;
+}
+// LOG_R fused stages starting at stage s on the group g of buffer b
+template <typename T, bool INVERSE, int LOG_R>
+__device__ __forceinline__ void radix_group(cx<T> *b, int g, int s, int N, const cx<T> *__restrict__ tw)
+{
+    constexpr int R = 1 << LOG_R;
+    const int pos = g & ((1 << s) - 1);
+    const int i0 = ((g >> s) << (s + LOG_R)) + pos;
+    cx<T> x[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) x[t] = b[i0 + (t << s)];
+#pragma unroll
+    for (int l = 0; l < LOG_R; ++l) {                  // stage s + l pairs local t and t + 2^l
+        const int tstride = (N >> 1) >> (s + l);
+#pragma unroll
+        for (int t = 0; t < R; ++t) {
+            if (t & (1 << l)) continue;
+            const int p = pos + ((t & ((1 << l) - 1)) << s);   // position of the pair inside its 2^(s+l+1) block
+            bfly<T, INVERSE>(x[t], x[t + (1 << l)], tw[p * tstride]);
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < R; ++t) b[i0 + (t << s)] = x[t];
+}
+template <typename T, bool INVERSE, int NBUF, int LOG_R>
+__device__ __forceinline__ void radix_pass(cx<T> *b0, cx<T> *b1, int s, int N, const cx<T> *__restrict__ tw)
+{
+    for (int g = threadIdx.x; g < (N >> LOG_R); g += blockDim.x) {
+        radix_group<T, INVERSE, LOG_R>(b0, g, s, N, tw);
+        if (NBUF == 2) radix_group<T, INVERSE, LOG_R>(b1, g, s, N, tw);
+    }
+    __syncthreads();
+}
 template <typename T, bool INVERSE, int NBUF>
 __device__ void cta_fft(cx<T> *b0, cx<T> *b1, int N, int logN, const cx<T> *__restrict__ tw)
 {
-    for (int s = 0; s < logN; ++s) {
-        const int half = 1 << s;
-        const int tstride = (N >> 1) >> s;
-        for (int j = threadIdx.x; j < (N >> 1); j += blockDim.x) {
-            const int pos = j & (half - 1);
-            const int i0 = ((j - pos) << 1) + pos;
-            const int i1 = i0 + half;
-            cx<T> w = tw[pos * tstride];
-            if (INVERSE) w.im = -w.im;
-            {
-                cx<T> a = b0[i0], t = cmul(w, b0[i1]);
-                b0[i0].re = a.re + t.re; b0[i0].im = a.im + t.im;
-                b0[i1].re = a.re - t.re; b0[i1].im = a.im - t.im;
-            }
-            if (NBUF == 2) {
-                cx<T> a = b1[i0], t = cmul(w, b1[i1]);
-                b1[i0].re = a.re + t.re; b1[i0].im = a.im + t.im;
-                b1[i1].re = a.re - t.re; b1[i1].im = a.im - t.im;
-            }
-        }
-        __syncthreads();
-    }
+    int s = 0;
+    const int r = logN % 3;
+    if (r == 1) { radix_pass<T, INVERSE, NBUF, 1>(b0, b1, 0, N, tw); s = 1; }
+    else if (r == 2) { radix_pass<T, INVERSE, NBUF, 2>(b0, b1, 0, N, tw); s = 2; }
+    for (; s < logN; s += 3) radix_pass<T, INVERSE, NBUF, 3>(b0, b1, s, N, tw);
 }
 
 // (value, index) max with lowest index on ties; every reduction stage uses the same rule.
