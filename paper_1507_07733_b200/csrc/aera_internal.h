@@ -116,9 +116,9 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
                               void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra = nullptr, int spec_mode = 0,
                               const UnfoldExt &x = UnfoldExt());
 
-// ---- unfold_t4k_f64.cu: team-per-station kernel for N = 4096 fp64, band rows 4..12 (configs[3])
-bool t4k_f64_supported(int dtype, const PlanDev &p);
-cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+// ---- unfold_t4k.cu: team-per-station kernel for N = 4096, fp64 (configs[3]) and fp32
+bool t4k_supported(int dtype, const PlanDev &p);
+cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                   void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x = UnfoldExt());
 
 // ---- unfold_long_f32.cu: multi-pass kernel for N = 65536 fp32 through an L2-resident scratch (configs[4])

@@ -501,7 +501,7 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     // up-sampling runs on the generic kernels (the specialised ones transform on the input grid only)
     const bool fast = kernel_variant() == 0 && ext.upsample == 1;
     const bool warp_path = fast && w32_supported(dtype, pl->dev);
-    const bool team_path = fast && !ext.input_i16 && t4k_f64_supported(dtype, pl->dev);
+    const bool team_path = fast && !ext.input_i16 && t4k_supported(dtype, pl->dev);
     const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
     const int layout = warp_path ? MINV_PACKED_PAD : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS));
     // complex elements of one event's matrices in this layout; the tables' slabs follow one another
@@ -521,12 +521,12 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
                         ws + w.off_minv + (size_t)t * x.minv_pattern_stride * cplx_bytes(dtype), layout, scale, s, forward, ext.g0, ext.g1);
     }
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
-    note_kernel(warp_path ? "unfold_w32" : (team_path ? "unfold_t4k_f64" : (long_path ? "unfold_long_f32" : "generic")));
+    note_kernel(warp_path ? "unfold_w32" : (team_path ? (dtype == AERA_F64 ? "unfold_t4k_f64" : "unfold_t4k_f32") : (long_path ? "unfold_long_f32" : "generic")));
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s,
                               spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode, x);
     else if (team_path)
-        e = launch_unfold_t4k_f64(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s, x);
+        e = launch_unfold_t4k(dtype, pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s, x);
     else if (long_path)
         e = launch_unfold_long_f32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv,
                                    ws + w.off_scratch, s, x);

@@ -50,6 +50,18 @@ struct LaneF64 {
     static __device__ __forceinline__ R fma(R a, R b, R c) { return __fma_rn(a, b, c); }
 };
 
+struct LaneF32 {   // plain float lanes (one transform), same code
+    using R = float;
+    using S = float;
+    static __device__ __forceinline__ R bc(S s) { return s; }
+    static __device__ __forceinline__ R zero() { return 0.0f; }
+    static __device__ __forceinline__ R neg(R a) { return -a; }
+    static __device__ __forceinline__ R add(R a, R b) { return __fadd_rn(a, b); }
+    static __device__ __forceinline__ R sub(R a, R b) { return __fsub_rn(a, b); }
+    static __device__ __forceinline__ R mul(R a, R b) { return __fmul_rn(a, b); }
+    static __device__ __forceinline__ R fma(R a, R b, R c) { return __fmaf_rn(a, b, c); }
+};
+
 template <int I> using IC = std::integral_constant<int, I>;
 template <int B, int E, class F>
 __device__ __forceinline__ void static_for(F &&f)

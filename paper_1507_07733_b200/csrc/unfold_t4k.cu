@@ -1,4 +1,5 @@
-// Team-per-station fused unfolding kernel for N = 4096 fp64 (BASELINE configs[3]).
+// Team-per-station fused unfolding kernel for N = 4096, fp64 (BASELINE configs[3]) and fp32 (the same code on plain
+// float lanes: a user with 4096-sample fp32 traces gets a register-resident path instead of the generic radix-8 one).
 //
 // A "team" of 4 warps (128 threads x 32 complex doubles = 128 registers each) holds one station
 // entirely in registers; a CTA runs 2 teams (8 warps, one CTA per SM, persistent). Every long
@@ -38,23 +39,44 @@
 namespace aera {
 namespace {
 
-using LD = LaneF64;
+// what differs between the two precisions: vector type, lane type for the 32-point FFT, global loads / stores
+template <typename T> struct T4k;
+template <> struct T4k<double> {
+    using T2 = double2; using Lane = LaneF64;
+    static __device__ __forceinline__ double ld_stream(const double *p) { double r; asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p)); return r; }
+    static __device__ __forceinline__ void st_stream(double *p, double v, unsigned long long pol) { asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory"); }
+    static __device__ __forceinline__ double2 ld_nc2(const double2 *p) { double2 r; asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p)); return r; }
+    static __device__ __forceinline__ unsigned long long bits(double v) { return (unsigned long long)__double_as_longlong(v); }
+    static __device__ __forceinline__ double from_bits(unsigned long long b) { return __longlong_as_double((long long)b); }
+    static __device__ __forceinline__ double2 make2(double a, double b) { return make_double2(a, b); }
+};
+template <> struct T4k<float> {
+    using T2 = float2; using Lane = LaneF32;
+    static __device__ __forceinline__ float ld_stream(const float *p) { float r; asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p)); return r; }
+    static __device__ __forceinline__ void st_stream(float *p, float v, unsigned long long pol) { asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(pol) : "memory"); }
+    static __device__ __forceinline__ float2 ld_nc2(const float2 *p) { float2 r; asm volatile("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p)); return r; }
+    static __device__ __forceinline__ unsigned long long bits(float v) { return (unsigned long long)__float_as_uint(v); }
+    static __device__ __forceinline__ float from_bits(unsigned long long b) { return __uint_as_float((unsigned)b); }
+    static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
+};
 constexpr int kTeams = 2;                             // 8 warps x 250 registers: no spills; a third team (168 registers) was 2 % slower
 constexpr int kTeamThreads = 128;
-constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane
+constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane (sized for fp64)
 constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B per team: exchange buffer / transpose planes / mirror rows
 constexpr int kTeamBytes = kRegionX;
 constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_4096^t, t < 1024)
 constexpr int kCtlF64 = 512;
 
+template <typename T>
 struct T4kParams {
-    const double *traces;
-    double *efield;
-    double *amp;
+    using T2 = typename T4k<T>::T2;
+    const T *traces;
+    T *efield;
+    T *amp;
     int32_t *idx;
-    const double2 *minv;   // [n_events] MINV_Q4 planes [q][entry][C] complex, scaled by 1/N
-    const double2 *tw1024; // W_1024^m
-    const double2 *twN;    // W_4096^m
+    const T2 *minv;   // [n_events] MINV_Q4 planes [q][entry][C] complex, scaled by 1/N
+    const T2 *tw1024; // W_1024^m
+    const T2 *twN;    // W_4096^m
     long n_units;
     int n_stations;
     int k_lo, k_hi, K;
@@ -66,12 +88,6 @@ __device__ __forceinline__ void team_sync(int team)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTeamThreads) : "memory");
 }
-__device__ __forceinline__ double ld_stream_f64(const double *p)
-{
-    double r;
-    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
-    return r;
-}
 // streamed output with an L2 evict_first policy: the written lines leave the L2 before the L2-prefetched traces do
 __device__ __forceinline__ unsigned long long t4k_policy_evict_first()
 {
@@ -79,23 +95,13 @@ __device__ __forceinline__ unsigned long long t4k_policy_evict_first()
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-__device__ __forceinline__ void st_stream_f64(double *p, double v, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
-}
-__device__ __forceinline__ double2 ld_nc_d2(const double2 *p)
-{
-    double2 r;
-    asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
-}
-
 // W_4096^t for any t in [0, 4096) from the first quadrant table: W^{t+1024} = -i W^t.
-__device__ __forceinline__ double2 w4096(const double2 *TQ, int t)
+template <typename T2>
+__device__ __forceinline__ T2 w4096(const T2 *TQ, int t)
 {
-    const double2 w = TQ[t & 1023];
+    const T2 w = TQ[t & 1023];
     const int quad = (t >> 10) & 3;
-    double2 r;
+    T2 r;
     r.x = (quad & 1) ? w.y : w.x;       // quad 1: -i w = (w.y, -w.x); quad 2: -w; quad 3: i w = (-w.y, w.x)
     r.y = (quad & 1) ? -w.x : w.y;
     if (quad & 2) { r.x = -r.x; r.y = -r.y; }
@@ -106,24 +112,26 @@ __device__ __forceinline__ double2 w4096(const double2 *TQ, int t)
 // sequence: two interleaved recurrences (even and odd k1, ratio W^{2 lane}) from TWO table reads
 // instead of 31. The shared-memory pipe, not the FP64 pipe, limits this kernel; 15 complex
 // multiplications per chain cost < 4e-15 of relative accuracy.
-__device__ __forceinline__ void pass_twiddle_d(double (&P)[32], double (&Q)[32], const double2 *__restrict__ T, int lane)
+template <typename T, typename T2>
+__device__ __forceinline__ void pass_twiddle_d(T (&P)[32], T (&Q)[32], const T2 *__restrict__ TW, int lane)
 {
-    const double2 w1 = T[32 + lane], w2 = T[64 + lane];     // W^{lane}, W^{2 lane}
-    double er = w2.x, ei = w2.y, orr = w1.x, oi = w1.y;      // current even / odd twiddle
+    const T2 w1 = TW[32 + lane], w2 = TW[64 + lane];     // W^{lane}, W^{2 lane}
+    T er = w2.x, ei = w2.y, orr = w1.x, oi = w1.y;      // current even / odd twiddle
     static_for<1, 32>([&](auto kc) {
         constexpr int k1 = decltype(kc)::value;
-        const double wr = (k1 & 1) ? orr : er, wi = (k1 & 1) ? oi : ei;
-        double a = P[k1] * wr; a = fma(Q[k1], -wi, a);
-        double b = P[k1] * wi; b = fma(Q[k1], wr, b);
+        const T wr = (k1 & 1) ? orr : er, wi = (k1 & 1) ? oi : ei;
+        T a = P[k1] * wr; a = fma(Q[k1], -wi, a);
+        T b = P[k1] * wi; b = fma(Q[k1], wr, b);
         P[k1] = a; Q[k1] = b;
         if constexpr (k1 + 2 < 32) {                         // advance the chain just used by W^{2 lane}
-            double nr = wr * w2.x; nr = fma(-wi, w2.y, nr);
-            double ni = wr * w2.y; ni = fma(wi, w2.x, ni);
+            T nr = wr * w2.x; nr = fma(-wi, w2.y, nr);
+            T ni = wr * w2.y; ni = fma(wi, w2.x, ni);
             if (k1 & 1) { orr = nr; oi = ni; } else { er = nr; ei = ni; }
         }
     });
 }
-__device__ __forceinline__ void transpose_plane_d(double (&P)[32], double *X, int lane)
+template <typename T>
+__device__ __forceinline__ void transpose_plane_d(T (&P)[32], T *X, int lane)
 {
     static_for<0, 32>([&](auto kc) {
         constexpr int k1 = decltype(kc)::value;
@@ -138,15 +146,16 @@ __device__ __forceinline__ void transpose_plane_d(double (&P)[32], double *X, in
 }
 // 1024-point forward FFT of in[brev5(j)] = x[lane + 32 j]; on return lane k1 holds X[k1 + 32 k2] in
 // (P[k2], Q[k2]). Call with (Q, P) for the un-normalised inverse. ONE copy of the 32-point code.
-__device__ __forceinline__ void fft1024_d(double (&P)[32], double (&Q)[32], double *X, const double2 *__restrict__ T, int lane)
+template <typename T, typename T2>
+__device__ __forceinline__ void fft1024_d(T (&P)[32], T (&Q)[32], T *X, const T2 *__restrict__ TW, int lane)
 {
     int second = 0;
     asm volatile("" : "+r"(second));
 #pragma unroll 1
     for (;;) {
-        fft32<LD>(P, Q);
+        fft32<typename T4k<T>::Lane>(P, Q);
         if (second) break;
-        pass_twiddle_d(P, Q, T, lane);
+        pass_twiddle_d(P, Q, TW, lane);
         transpose_plane_d(P, X, lane);
         transpose_plane_d(Q, X, lane);
         second = 1;
@@ -154,32 +163,34 @@ __device__ __forceinline__ void fft1024_d(double (&P)[32], double (&Q)[32], doub
     }
 }
 
-template <int RLO, int RHI, bool HAS_EF>
+template <typename T, int RLO, int RHI, bool HAS_EF>
 __global__ void __launch_bounds__(kTeams *kTeamThreads, 1)
-unfold_t4k_f64_kernel(T4kParams p)
+unfold_t4k_kernel(T4kParams<T> p)
 {
+    using T2 = typename T4k<T>::T2;
+    using K = T4k<T>;
     constexpr int kRows = RHI - RLO + 1;            // band rows per thread
     static_assert(kRows >= 1 && kRows <= 16, "band rows of 128 bins below N/2");
     constexpr int kMirLo = 31 - RHI, kMirHi = (32 - RLO) > 31 ? 31 : (32 - RLO); // rows holding some band bin's mirror
     constexpr int kMirRows = kMirHi - kMirLo + 1;
     static_assert(4 * kMirRows * 512 <= kRegionX, "mirror rows fit region X");
     extern __shared__ __align__(128) unsigned char smem[];
-    double2 *T = reinterpret_cast<double2 *>(smem);        // [32][32] pass twiddles W_1024^{k1 t}
-    double2 *TQ = T + 1024;                                 // W_4096^t, t < 1024
+    T2 *TW = reinterpret_cast<T2 *>(smem);        // [32][32] pass twiddles W_1024^{k1 t}
+    T2 *TQ = TW + 1024;                                 // W_4096^t, t < 1024
     uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabF64);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
     const int team = warp >> 2, w = warp & 3;
-    double *peak_v = reinterpret_cast<double *>(smem + kTabF64 + 64) + team * 4;   // [team][4]
+    T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + team * 4;   // [team][4]
     int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + kTeams * 32) + team * 4;
     unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kTeamBytes;
-    double *RX = reinterpret_cast<double *>(tb);            // region X
-    double *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
+    T *RX = reinterpret_cast<T *>(tb);            // region X
+    T *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
 
     if (warp == 0) tmem_alloc_all(tmem_base);
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
         const int k1 = i >> 5, t = i & 31;
-        T[i] = p.tw1024[(k1 * t) & 1023];
+        TW[i] = p.tw1024[(k1 * t) & 1023];
         TQ[i] = p.twN[i];
     }
     tmem_fence_before_sync();
@@ -195,33 +206,33 @@ unfold_t4k_f64_kernel(T4kParams p)
 
 #pragma unroll 1
     for (long u = u0 + team; u < u1; u += kTeams) {
-        const double *v = p.traces + (size_t)u * 2 * N;
-        double *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
+        const T *v = p.traces + (size_t)u * 2 * N;
+        T *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
         const long ev = u / p.n_stations;
-        const double2 *M = p.minv + (size_t)ev * minv_q4_stride(p.k_lo, p.k_hi) +
+        const T2 *M = p.minv + (size_t)ev * minv_q4_stride(p.k_lo, p.k_hi) +
                            (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
-        if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(double));
+        if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(T));
 
-        double P[32], Q[32];
+        T P[32], Q[32];
         // ---- a1 + radix-4 step: thread holds y_q[m], q = 0..3, m = lane + 32 (8 w + jj), at [8 q + jj]
         static_for<0, 8>([&](auto jc) {
             constexpr int jj = decltype(jc)::value;
             const int m = lane + 32 * (8 * w + jj);
-            const double x0r = ld_stream_f64(v + m), x1r = ld_stream_f64(v + m + 1024);
-            const double x2r = ld_stream_f64(v + m + 2048), x3r = ld_stream_f64(v + m + 3072);
-            const double x0i = ld_stream_f64(v + N + m), x1i = ld_stream_f64(v + N + m + 1024);
-            const double x2i = ld_stream_f64(v + N + m + 2048), x3i = ld_stream_f64(v + N + m + 3072);
-            const double ar = x0r + x2r, ai = x0i + x2i, br = x0r - x2r, bi = x0i - x2i;
-            const double cr = x1r + x3r, ci = x1i + x3i, dr = x1r - x3r, di = x1i - x3i;
+            const T x0r = K::ld_stream(v + m), x1r = K::ld_stream(v + m + 1024);
+            const T x2r = K::ld_stream(v + m + 2048), x3r = K::ld_stream(v + m + 3072);
+            const T x0i = K::ld_stream(v + N + m), x1i = K::ld_stream(v + N + m + 1024);
+            const T x2i = K::ld_stream(v + N + m + 2048), x3i = K::ld_stream(v + N + m + 3072);
+            const T ar = x0r + x2r, ai = x0i + x2i, br = x0r - x2r, bi = x0i - x2i;
+            const T cr = x1r + x3r, ci = x1i + x3i, dr = x1r - x3r, di = x1i - x3i;
             P[jj] = ar + cr; Q[jj] = ai + ci;                    // y0
-            const double y1r = br + di, y1i = bi - dr;           // b - i d
-            const double y2r = ar - cr, y2i = ai - ci;
-            const double y3r = br - di, y3i = bi + dr;           // b + i d
-            const double2 w1 = TQ[m];                            // W_4096^m, m < 1024
-            double2 w2, w3;                                      // W^{2m}, W^{3m} by multiplication: one table read, not three
+            const T y1r = br + di, y1i = bi - dr;           // b - i d
+            const T y2r = ar - cr, y2i = ai - ci;
+            const T y3r = br - di, y3i = bi + dr;           // b + i d
+            const T2 w1 = TQ[m];                            // W_4096^m, m < 1024
+            T2 w2, w3;                                      // W^{2m}, W^{3m} by multiplication: one table read, not three
             w2.x = fma(w1.x, w1.x, -(w1.y * w1.y)); w2.y = (w1.x + w1.x) * w1.y;
             w3.x = fma(w2.x, w1.x, -(w2.y * w1.y)); w3.y = fma(w2.x, w1.y, w2.y * w1.x);
-            double t;
+            T t;
             t = y1r * w1.x; P[8 + jj] = fma(y1i, -w1.y, t); t = y1r * w1.y; Q[8 + jj] = fma(y1i, w1.x, t);
             t = y2r * w2.x; P[16 + jj] = fma(y2i, -w2.y, t); t = y2r * w2.y; Q[16 + jj] = fma(y2i, w2.x, t);
             t = y3r * w3.x; P[24 + jj] = fma(y3i, -w3.y, t); t = y3r * w3.y; Q[24 + jj] = fma(y3i, w3.x, t);
@@ -230,7 +241,7 @@ unfold_t4k_f64_kernel(T4kParams p)
         // ---- team exchange: warp q collects y_q[lane + 32 j], j = 8 w' + jj, into FFT input order
         team_sync(team);                                         // region X free (previous station done)
         {
-            double *XB = RX;                                     // [q][j][lane]
+            T *XB = RX;                                     // [q][j][lane]
             static_for<0, 32>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;           // i = 8 q + jj
                 XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane] = P[i];
@@ -253,25 +264,25 @@ unfold_t4k_f64_kernel(T4kParams p)
             team_sync(team);
         }
         // ---- a2: warp q = w: G[4 (lane + 32 row) + q] in (P[row], Q[row])
-        fft1024_d(P, Q, XW, T, lane);
+        fft1024_d(P, Q, XW, TW, lane);
         team_sync(team);                                         // all transposes done: region X becomes the mirror rows
         {
-            double2 *PUB = reinterpret_cast<double2 *>(RX);      // [warp][mirror row][lane]
+            T2 *PUB = reinterpret_cast<T2 *>(RX);      // [warp][mirror row][lane]
             static_for<kMirLo, kMirHi + 1>([&](auto rc) {
                 constexpr int r = decltype(rc)::value;
-                PUB[(w * kMirRows + (r - kMirLo)) * 32 + lane] = make_double2(P[r], Q[r]);
+                PUB[(w * kMirRows + (r - kMirLo)) * 32 + lane] = K::make2(P[r], Q[r]);
             });
         }
         team_sync(team);
         // ---- separation + a4 on the band rows: E for this warp's bins k = 4 (lane + 32 r) + w, in registers
-        double Etr[kRows], Eti[kRows];
+        T Etr[kRows], Eti[kRows];
         {
-            const double2 *PUB = reinterpret_cast<const double2 *>(RX);
+            const T2 *PUB = reinterpret_cast<const T2 *>(RX);
             const int pw = (4 - w) & 3;
             const int plane = (w == 0) ? ((32 - lane) & 31) : (31 - lane);
             const int padd = (w == 0 && lane == 0) ? 1 : 0;      // q = 0, lane 0: mirror row 32 - r
             const int C = (p.k_hi >> 2) - (p.k_lo >> 2) + 1;     // Minv columns per (q, entry) plane
-            const double2 *Mq = M + (size_t)w * 4 * C;
+            const T2 *Mq = M + (size_t)w * 4 * C;
             static_for<0, kRows>([&](auto rc) {
                 constexpr int i = decltype(rc)::value;
                 constexpr int r = RLO + i;
@@ -279,21 +290,21 @@ unfold_t4k_f64_kernel(T4kParams p)
                 const bool inband = k >= p.k_lo && k <= p.k_hi;
                 int prow = 31 - r + padd;
                 prow = prow > kMirHi ? kMirHi : prow;
-                const double2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
+                const T2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
                 int c = lane + 32 * r - (p.k_lo >> 2);
                 c = c < 0 ? 0 : (c > C - 1 ? C - 1 : c);
-                const double2 m0 = ld_nc_d2(Mq + c), m1 = ld_nc_d2(Mq + C + c);
-                const double2 m2 = ld_nc_d2(Mq + 2 * C + c), m3 = ld_nc_d2(Mq + 3 * C + c);
-                const double v0r = P[r] + gm.x, v0i = Q[r] - gm.y;   // 2 V_0
-                const double v1r = Q[r] + gm.y, v1i = gm.x - P[r];   // 2 V_1
-                double er = m0.x * v0r; er = fma(-m0.y, v0i, er); er = fma(m1.x, v1r, er); er = fma(-m1.y, v1i, er);
-                double ei = m0.x * v0i; ei = fma(m0.y, v0r, ei); ei = fma(m1.x, v1i, ei); ei = fma(m1.y, v1r, ei);
-                double fr = m2.x * v0r; fr = fma(-m2.y, v0i, fr); fr = fma(m3.x, v1r, fr); fr = fma(-m3.y, v1i, fr);
-                double fi = m2.x * v0i; fi = fma(m2.y, v0r, fi); fi = fma(m3.x, v1i, fi); fi = fma(m3.y, v1r, fi);
-                Etr[i] = inband ? er : 0.0; Eti[i] = inband ? ei : 0.0;
+                const T2 m0 = K::ld_nc2(Mq + c), m1 = K::ld_nc2(Mq + C + c);
+                const T2 m2 = K::ld_nc2(Mq + 2 * C + c), m3 = K::ld_nc2(Mq + 3 * C + c);
+                const T v0r = P[r] + gm.x, v0i = Q[r] - gm.y;   // 2 V_0
+                const T v1r = Q[r] + gm.y, v1i = gm.x - P[r];   // 2 V_1
+                T er = m0.x * v0r; er = fma(-m0.y, v0i, er); er = fma(m1.x, v1r, er); er = fma(-m1.y, v1i, er);
+                T ei = m0.x * v0i; ei = fma(m0.y, v0r, ei); ei = fma(m1.x, v1i, ei); ei = fma(m1.y, v1r, ei);
+                T fr = m2.x * v0r; fr = fma(-m2.y, v0i, fr); fr = fma(m3.x, v1r, fr); fr = fma(-m3.y, v1i, fr);
+                T fi = m2.x * v0i; fi = fma(m2.y, v0r, fi); fi = fma(m3.x, v1i, fi); fi = fma(m3.y, v1r, fi);
+                Etr[i] = inband ? er : (T)0; Eti[i] = inband ? ei : (T)0;
                 // E_phi waits in tensor memory while the registers hold the theta transform
-                tmem_st64(tephi + 4 * i, (unsigned long long)__double_as_longlong(inband ? fr : 0.0));
-                tmem_st64(tephi + 4 * i + 2, (unsigned long long)__double_as_longlong(inband ? fi : 0.0));
+                tmem_st64(tephi + 4 * i, K::bits(inband ? fr : (T)0));
+                tmem_st64(tephi + 4 * i + 2, K::bits(inband ? fi : (T)0));
             });
         }
         team_sync(team);                                         // mirror rows consumed: region X is free for transposes
@@ -302,13 +313,13 @@ unfold_t4k_f64_kernel(T4kParams p)
         // bins Z[4 k' + q] (zero outside the band rows), multiplies by W_4096^{-m q}, the team exchanges,
         // and the radix-4 step gives z[m + 1024 s], s = 0..3, for this thread's 8 values of m:
         // contiguous 8-byte stores, 256 bytes per warp instruction.
-        double best = -1.0; int bn = 0;
+        T best = (T)-1; int bn = 0;
 #pragma unroll 1
         for (int pol = 0; pol < 2; ++pol) {
             if (pol == 0) {
                 static_for<0, 32>([&](auto kc) {
                     constexpr int r = decltype(kc)::value;
-                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = 0.0; Q[brev5(r)] = 0.0; }
+                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = (T)0; Q[brev5(r)] = (T)0; }
                     else { P[brev5(r)] = Etr[r - RLO]; Q[brev5(r)] = Eti[r - RLO]; }
                 });
             } else {
@@ -325,36 +336,36 @@ unfold_t4k_f64_kernel(T4kParams p)
                 });
                 static_for<0, 32>([&](auto kc) {
                     constexpr int r = decltype(kc)::value;
-                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = 0.0; Q[brev5(r)] = 0.0; }
+                    if constexpr (r < RLO || r > RHI) { P[brev5(r)] = (T)0; Q[brev5(r)] = (T)0; }
                     else {
-                        P[brev5(r)] = __longlong_as_double((long long)ev[2 * (r - RLO)]);
-                        Q[brev5(r)] = __longlong_as_double((long long)ev[2 * (r - RLO) + 1]);
+                        P[brev5(r)] = K::from_bits(ev[2 * (r - RLO)]);
+                        Q[brev5(r)] = K::from_bits(ev[2 * (r - RLO) + 1]);
                     }
                 });
             }
-            fft1024_d(Q, P, XW, T, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
+            fft1024_d(Q, P, XW, TW, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
             if (w != 0) {
                 // u_q[m] conj(W_4096^{q m}), m = lane + 32 b: two interleaved recurrences over b (ratio W^{64 q})
-                const double2 r2 = w4096(TQ, 64 * w);
-                const double2 c0 = w4096(TQ, (w * lane) & 4095), c1 = w4096(TQ, (w * (lane + 32)) & 4095);
-                double er = c0.x, ei = c0.y, orr = c1.x, oi = c1.y;
+                const T2 r2 = w4096(TQ, 64 * w);
+                const T2 c0 = w4096(TQ, (w * lane) & 4095), c1 = w4096(TQ, (w * (lane + 32)) & 4095);
+                T er = c0.x, ei = c0.y, orr = c1.x, oi = c1.y;
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
-                    const double wr = (b & 1) ? orr : er, wi = (b & 1) ? oi : ei;
-                    const double ur = P[b], ui = Q[b];
-                    double a = ur * wr; a = fma(ui, wi, a);
-                    double c = ui * wr; c = fma(ur, -wi, c);
+                    const T wr = (b & 1) ? orr : er, wi = (b & 1) ? oi : ei;
+                    const T ur = P[b], ui = Q[b];
+                    T a = ur * wr; a = fma(ui, wi, a);
+                    T c = ui * wr; c = fma(ur, -wi, c);
                     P[b] = a; Q[b] = c;
                     if constexpr (b + 2 < 32) {
-                        double nr = wr * r2.x; nr = fma(-wi, r2.y, nr);
-                        double ni = wr * r2.y; ni = fma(wi, r2.x, ni);
+                        T nr = wr * r2.x; nr = fma(-wi, r2.y, nr);
+                        T ni = wr * r2.y; ni = fma(wi, r2.x, ni);
                         if (b & 1) { orr = nr; oi = ni; } else { er = nr; ei = ni; }
                     }
                 });
             }
             team_sync(team);                                     // all transposes done: region X is the exchange buffer
             {
-                double *XB = RX;                                 // [q][b][lane]
+                T *XB = RX;                                 // [q][b][lane]
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
                     XB[(w * 32 + b) * 32 + lane] = P[b];
@@ -379,10 +390,10 @@ unfold_t4k_f64_kernel(T4kParams p)
             // radix-4 step (inverse sign): z_s = sum_q (+i)^{s q} u_q, left in place at [8 s + jj]
             static_for<0, 8>([&](auto jc) {
                 constexpr int jj = decltype(jc)::value;
-                const double ar = P[jj] + P[16 + jj], ai = Q[jj] + Q[16 + jj];
-                const double br = P[jj] - P[16 + jj], bi = Q[jj] - Q[16 + jj];
-                const double cr = P[8 + jj] + P[24 + jj], ci = Q[8 + jj] + Q[24 + jj];
-                const double dr = P[8 + jj] - P[24 + jj], di = Q[8 + jj] - Q[24 + jj];
+                const T ar = P[jj] + P[16 + jj], ai = Q[jj] + Q[16 + jj];
+                const T br = P[jj] - P[16 + jj], bi = Q[jj] - Q[16 + jj];
+                const T cr = P[8 + jj] + P[24 + jj], ci = Q[8 + jj] + Q[24 + jj];
+                const T dr = P[8 + jj] - P[24 + jj], di = Q[8 + jj] - Q[24 + jj];
                 P[jj] = ar + cr; Q[jj] = ai + ci;
                 P[8 + jj] = br - di; Q[8 + jj] = bi + dr;        // b + i d
                 P[16 + jj] = ar - cr; Q[16 + jj] = ai - ci;
@@ -393,9 +404,9 @@ unfold_t4k_f64_kernel(T4kParams p)
             if (pol == 0) {
                 static_for<0, 32>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    if (HAS_EF) st_stream_f64(ef + nbase + 32 * (i & 7) + 1024 * (i >> 3), P[i], pol_first);
-                    double e2 = P[i] * P[i]; e2 = fma(Q[i], Q[i], e2);
-                    tmem_st64(tenv + 2 * i, (unsigned long long)__double_as_longlong(e2));
+                    if (HAS_EF) K::st_stream(ef + nbase + 32 * (i & 7) + 1024 * (i >> 3), P[i], pol_first);
+                    T e2 = P[i] * P[i]; e2 = fma(Q[i], Q[i], e2);
+                    tmem_st64(tenv + 2 * i, K::bits(e2));
                 });
                 tmem_wait_st();
             } else {
@@ -415,8 +426,8 @@ unfold_t4k_f64_kernel(T4kParams p)
                         constexpr int j = decltype(jc)::value;
                         constexpr int i = 8 * c + j;
                         const int n = nbase + 32 * (i & 7) + 1024 * (i >> 3);
-                        if (HAS_EF) st_stream_f64(ef + N + n, P[i], pol_first);
-                        double e2 = fma(P[i], P[i], __longlong_as_double((long long)ev[j]));
+                        if (HAS_EF) K::st_stream(ef + N + n, P[i], pol_first);
+                        T e2 = fma(P[i], P[i], K::from_bits(ev[j]));
                         e2 = fma(Q[i], Q[i], e2);
                         if (e2 > best) { best = e2; bn = n; }
                     });
@@ -427,14 +438,14 @@ unfold_t4k_f64_kernel(T4kParams p)
         int bi = bn;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const T ob = __shfl_xor_sync(0xffffffffu, best, o);
             const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
             if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
         }
         if (lane == 0) { peak_v[w] = best; peak_i[w] = bi; }
         team_sync(team);
         if (w == 0 && lane == 0) {
-            double bv = peak_v[0]; int bx = peak_i[0];
+            T bv = peak_v[0]; int bx = peak_i[0];
 #pragma unroll
             for (int i = 1; i < 4; ++i)
                 if (peak_v[i] > bv || (peak_v[i] == bv && peak_i[i] < bx)) { bv = peak_v[i]; bx = peak_i[i]; }
@@ -446,11 +457,11 @@ unfold_t4k_f64_kernel(T4kParams p)
     if (warp == 0) tmem_free_all(*tmem_base);
 }
 
-template <int RLO, int RHI, bool HAS_EF>
-cudaError_t launch_t4k(const T4kParams &q, cudaStream_t s)
+template <typename T, int RLO, int RHI, bool HAS_EF>
+cudaError_t launch_t4k(const T4kParams<T> &q, cudaStream_t s)
 {
     const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * kTeamBytes;
-    auto kern = unfold_t4k_f64_kernel<RLO, RHI, HAS_EF>;
+    auto kern = unfold_t4k_kernel<T, RLO, RHI, HAS_EF>;
     AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + kTeams - 1) / kTeams;
     if (grid > sm_count()) grid = sm_count();
@@ -458,28 +469,36 @@ cudaError_t launch_t4k(const T4kParams &q, cudaStream_t s)
     return cudaGetLastError();
 }
 
-} // namespace
-
-bool t4k_f64_supported(int dtype, const PlanDev &p)
+template <typename T>
+cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield, void *amp, int32_t *idx,
+                             const void *minv, cudaStream_t s, const UnfoldExt &x)
 {
+    using T2 = typename T4k<T>::T2;
+    T4kParams<T> q;
+    q.traces = (const T *)traces; q.efield = (T *)efield; q.amp = (T *)amp; q.idx = idx;
+    q.minv = (const T2 *)minv; q.tw1024 = (const T2 *)p.tw1024; q.twN = (const T2 *)p.twN;
+    q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
+    q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
     // rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3]) have their own instantiation; <0, 15> serves any other band
-    return dtype == AERA_F64 && p.N == 4096 && p.k_lo >= 1 && p.k_hi < 2048;
+    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) return efield ? launch_t4k<T, 4, 12, true>(q, s) : launch_t4k<T, 4, 12, false>(q, s);
+    return efield ? launch_t4k<T, 0, 15, true>(q, s) : launch_t4k<T, 0, 15, false>(q, s);
 }
 
-cudaError_t launch_unfold_t4k_f64(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
-                                  void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x)
+} // namespace
+
+bool t4k_supported(int dtype, const PlanDev &p)
+{
+    return (dtype == AERA_F64 || dtype == AERA_F32) && p.N == 4096 && p.k_lo >= 1 && p.k_hi < 2048;
+}
+
+cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
+                              void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x)
 {
     const long n_units = n_events * (long)n_stations;
     if (n_units <= 0) return cudaSuccess;
     ProfScope prof(KID_UNFOLD, s);
-    T4kParams q;
-    q.traces = (const double *)traces; q.efield = (double *)efield; q.amp = (double *)amp; q.idx = idx;
-    q.minv = (const double2 *)minv; q.tw1024 = (const double2 *)p.tw1024; q.twN = (const double2 *)p.twN;
-    q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
-    q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
-    cudaError_t e;
-    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) e = efield ? launch_t4k<4, 12, true>(q, s) : launch_t4k<4, 12, false>(q, s);
-    else e = efield ? launch_t4k<0, 15, true>(q, s) : launch_t4k<0, 15, false>(q, s);
+    const cudaError_t e = dtype == AERA_F64 ? launch_t4k_typed<double>(p, n_units, n_stations, traces, efield, amp, idx, minv, s, x)
+                                            : launch_t4k_typed<float>(p, n_units, n_stations, traces, efield, amp, idx, minv, s, x);
     count_launches(1);
     return e;
 }

@@ -19,6 +19,7 @@ def B():
 
 @pytest.mark.parametrize("dtype,N,fs,kernel", [("f32", 2048, 200e6, "unfold_w32"), ("f32", 2048, 250e6, "unfold_w32"),
                                                ("f64", 4096, 250e6, "unfold_t4k_f64"), ("f64", 4096, 180e6, "unfold_t4k_f64"),
+                                               ("f32", 4096, 200e6, "unfold_t4k_f32"), ("f32", 4096, 250e6, "unfold_t4k_f32"),
                                                ("f32", 1024, 200e6, "generic"), ("f64", 2048, 200e6, "generic")])
 def test_batch_other_bands(B, dtype, N, fs, kernel):
     import oracle
