@@ -59,7 +59,8 @@ template <> struct T4k<float> {
     static __device__ __forceinline__ float from_bits(unsigned long long b) { return __uint_as_float((unsigned)b); }
     static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
 };
-constexpr int kTeams = 2;                             // 8 warps x 250 registers: no spills; a third team (168 registers) was 2 % slower
+// teams per CTA: 2 in fp64 (8 warps x 250 registers; a third team, 168 registers, gains nothing), 4 in fp32 (16 warps x 128)
+template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? 2 : 4;
 constexpr int kTeamThreads = 128;
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane (sized for fp64)
 constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B per team: exchange buffer / transpose planes / mirror rows
@@ -163,7 +164,7 @@ __device__ __forceinline__ void fft1024_d(T (&P)[32], T (&Q)[32], T *X, const T2
     }
 }
 
-template <typename T, int RLO, int RHI, bool HAS_EF>
+template <typename T, int RLO, int RHI, bool HAS_EF, int kTeams>
 __global__ void __launch_bounds__(kTeams *kTeamThreads, 1)
 unfold_t4k_kernel(T4kParams<T> p)
 {
@@ -460,8 +461,9 @@ unfold_t4k_kernel(T4kParams<T> p)
 template <typename T, int RLO, int RHI, bool HAS_EF>
 cudaError_t launch_t4k(const T4kParams<T> &q, cudaStream_t s)
 {
+    constexpr int kTeams = kTeamsOf<T>;
     const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * kTeamBytes;
-    auto kern = unfold_t4k_kernel<T, RLO, RHI, HAS_EF>;
+    auto kern = unfold_t4k_kernel<T, RLO, RHI, HAS_EF, kTeams>;
     AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + kTeams - 1) / kTeams;
     if (grid > sm_count()) grid = sm_count();
