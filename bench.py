@@ -435,11 +435,18 @@ def main():
     ap.add_argument("--peaks", action="store_true", help="measure and print the device's ALU issue peaks (packed fp32, fp32, fp64) and exit")
     ap.add_argument("--i16", action="store_true", help="int16 ADC-count input (aera_unfold_batch_i16): 24 584 algorithmic bytes per unit at configs[1]")
     ap.add_argument("--patterns", type=int, default=1, help="number of resident antenna-pattern tables, stations assigned round-robin (aera_unfold_batch_multi)")
+    ap.add_argument("--fs-mhz", type=float, default=0.0, help="variant of the config at another sampling rate (another band-row geometry; not a BASELINE workload)")
+    ap.add_argument("--samples", type=int, default=0, help="variant of the config at another trace length (not a BASELINE workload)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     wl = ai.WORKLOADS[args.config]
+    if args.fs_mhz > 0 or args.samples > 0:
+        import dataclasses
+        n = args.samples or wl.n_samples
+        wl = dataclasses.replace(wl, name=wl.name + f" VARIANT fs={args.fs_mhz or wl.fs_hz / 1e6:g} MHz N={n}", fs_hz=args.fs_mhz * 1e6 if args.fs_mhz > 0 else wl.fs_hz,
+                                 n_samples=n, arrival_lo=n // 4, arrival_hi=3 * n // 4)
 
     if args.impl == "reference":
         run_reference(args, wl)

@@ -81,16 +81,17 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
 //                 B = {t1.re, p1.re, t1.im, p1.im}                                     (warp kernels)
 //   MINV_Q4     : per direction 16 planes [q = k & 3][entry 0..3 as in MINV_ROWS][C] complex, column
 //                 (k >> 2) - (k_lo >> 2), C = (k_hi >> 2) - (k_lo >> 2) + 1; slots of bins outside the
-//                 band are never written or used                                       (team kernel)
+//                 band are never written or used                                       (team kernel, teams of 4 warps)
+//   MINV_Q2, MINV_Q1 : the same with q = k & 1 (8 planes) / q = 0 (4 planes, C = K)    (teams of 2 warps / 1 warp)
 //   MINV_Q32    : per direction 64 float4 planes [q = k & 31][A | B as in MINV_PACKED][C], column
 //                 (k >> 5) - (k_lo >> 5), C = (k_hi >> 5) - (k_lo >> 5) + 1              (long-trace kernel)
 //   MINV_PACKED_PAD : MINV_PACKED with 32 zero entries before and after each plane (planes of K + 64 entries, bin j at
 //                 index j + 32): a warp kernel whose edge rows reach up to 31 bins beyond the band multiplies by zero
 //                 there instead of clamping the index and selecting                       (batch warp kernel)
-enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3, MINV_PACKED_PAD = 4 };
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3, MINV_PACKED_PAD = 4, MINV_Q2 = 5, MINV_Q1 = 6 };
 constexpr int kMinvPad = 32;
-// complex elements per direction in the MINV_Q4 layout (<= 4 K + 32)
-__host__ __device__ inline size_t minv_q4_stride(int k_lo, int k_hi) { return (size_t)16 * ((k_hi >> 2) - (k_lo >> 2) + 1); }
+// complex elements per direction in the MINV_Q4 / Q2 / Q1 layouts, tw = 4 / 2 / 1 (<= 4 K + 8 tw)
+__host__ __device__ inline size_t minv_qt_stride(int tw, int k_lo, int k_hi) { return (size_t)4 * tw * ((k_hi / tw) - (k_lo / tw) + 1); }
 cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const PlanDev &p,
                         const double *dirs, long n_dirs, void *minv, int layout, double scale, cudaStream_t s,
                         int forward = 0 /* 1: scale * H (forward model) instead of scale * H^-1 */,
@@ -116,8 +117,9 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
                               void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra = nullptr, int spec_mode = 0,
                               const UnfoldExt &x = UnfoldExt());
 
-// ---- unfold_t4k.cu: team-per-station kernel for N = 4096, fp64 (configs[3]) and fp32
+// ---- unfold_t4k.cu: team-per-station kernel, N = 1024 x (warps of a team): 4096 fp64 (configs[3]) / fp32, 2048 fp64, 1024 fp64 / fp32
 bool t4k_supported(int dtype, const PlanDev &p);
+int t4k_team_warps(int dtype, const PlanDev &p);   // 4, 2, 1, or 0 when the kernel does not cover (dtype, N, band)
 cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                   void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x = UnfoldExt());
 

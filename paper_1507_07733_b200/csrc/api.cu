@@ -336,6 +336,12 @@ aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches)
 
 const char *aera_last_error(void) { return g_err; }
 const char *aera_last_kernel(void) { return g_last_kernel; }
+static const char *team_kernel_name(int dtype, int team_warps)
+{
+    if (team_warps == 4) return dtype == AERA_F64 ? "unfold_t4k_f64" : "unfold_t4k_f32";
+    if (team_warps == 2) return dtype == AERA_F64 ? "unfold_t2k_f64" : "unfold_t2k_f32";
+    return dtype == AERA_F64 ? "unfold_t1k_f64" : "unfold_t1k_f32";
+}
 
 aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count_out, int *sm_clock_khz)
 {
@@ -503,9 +509,11 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     const bool warp_path = fast && w32_supported(dtype, pl->dev);
     const bool team_path = fast && !ext.input_i16 && t4k_supported(dtype, pl->dev);
     const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
-    const int layout = warp_path ? MINV_PACKED_PAD : (team_path ? MINV_Q4 : (long_path ? MINV_Q32 : MINV_ROWS));
+    const int team_warps = team_path ? t4k_team_warps(dtype, pl->dev) : 0;
+    const int layout = warp_path ? MINV_PACKED_PAD
+                                 : (team_path ? (team_warps == 4 ? MINV_Q4 : (team_warps == 2 ? MINV_Q2 : MINV_Q1)) : (long_path ? MINV_Q32 : MINV_ROWS));
     // complex elements of one event's matrices in this layout; the tables' slabs follow one another
-    const size_t per_event = layout == MINV_Q4 ? minv_q4_stride(pl->dev.k_lo, pl->dev.k_hi)
+    const size_t per_event = team_path ? minv_qt_stride(team_warps, pl->dev.k_lo, pl->dev.k_hi)
                              : (layout == MINV_Q32 ? (size_t)128 * ((pl->dev.k_hi >> 5) - (pl->dev.k_lo >> 5) + 1)
                                                    : (layout == MINV_PACKED_PAD ? (size_t)(pl->dev.K + 2 * kMinvPad) * 4 : (size_t)pl->dev.K * 4));
     UnfoldExt x;
@@ -521,7 +529,7 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
                         ws + w.off_minv + (size_t)t * x.minv_pattern_stride * cplx_bytes(dtype), layout, scale, s, forward, ext.g0, ext.g1);
     }
     if (e != cudaSuccess) return cuda_fail(e, "minv kernel launch");
-    note_kernel(warp_path ? "unfold_w32" : (team_path ? (dtype == AERA_F64 ? "unfold_t4k_f64" : "unfold_t4k_f32") : (long_path ? "unfold_long_f32" : "generic")));
+    note_kernel(warp_path ? "unfold_w32" : (team_path ? team_kernel_name(dtype, team_warps) : (long_path ? "unfold_long_f32" : "generic")));
     if (warp_path)
         e = launch_unfold_w32(pl->dev, n_events, n_stations, traces, efield, peak_amp, peak_idx, ws + w.off_minv, s,
                               spec_mode ? ws + w.off_loop_spectra : nullptr, spec_mode, x);

@@ -1,5 +1,8 @@
 // Team-per-station fused unfolding kernel for N = 4096, fp64 (BASELINE configs[3]) and fp32 (the same code on plain
 // float lanes: a user with 4096-sample fp32 traces gets a register-resident path instead of the generic radix-8 one).
+// The team size TW is a template parameter: N = 1024 TW, TW = 4 (described below), 2 (N = 2048: a radix-2 step across
+// two warps) or 1 (N = 1024: one warp per station, no team exchange), so fp64 traces of 1024 / 2048 samples and fp32
+// traces of 1024 samples stay register-resident too (fp32 N = 2048 is unfold_w32.cu's).
 //
 // A "team" of 4 warps (128 threads x 32 complex doubles = 128 registers each) holds one station
 // entirely in registers; a CTA runs 2 teams (8 warps, one CTA per SM, persistent). Every long
@@ -60,13 +63,15 @@ template <> struct T4k<float> {
     static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
 };
 // teams per CTA: 2 in fp64 (8 warps x 250 registers; a third team, 168 registers, gains nothing), 4 in fp32 (16 warps x 128)
-template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? 2 : 4;
-constexpr int kTeamThreads = 128;
+#ifndef AERA_T4K_TEAMS_F64
+#define AERA_T4K_TEAMS_F64 2
+#endif
+// (TW < 4: the same number of warps per CTA, i.e. 4 / TW times the teams)
+template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? AERA_T4K_TEAMS_F64 : 4;
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane (sized for fp64)
-constexpr int kRegionX = 4 * kPlaneBytes;             // 33 792 B per team: exchange buffer / transpose planes / mirror rows
-constexpr int kTeamBytes = kRegionX;
-constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_4096^t, t < 1024)
-constexpr int kCtlF64 = 512;
+// region X of a team = TW planes (33 792 B at TW = 4): exchange buffer / transpose planes / mirror rows
+constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_N^t, t < 1024)
+constexpr int kCtlF64 = 1024;                         // TMEM base, per-team peak slots (up to 16 teams)
 
 template <typename T>
 struct T4kParams {
@@ -85,9 +90,11 @@ struct T4kParams {
     size_t minv_pattern_stride;  // double2 elements between the Minv slabs of consecutive tables
 };
 
+template <int TW>
 __device__ __forceinline__ void team_sync(int team)
 {
-    asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTeamThreads) : "memory");
+    if constexpr (TW == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(TW * 32) : "memory");
 }
 // streamed output with an L2 evict_first policy: the written lines leave the L2 before the L2-prefetched traces do
 __device__ __forceinline__ unsigned long long t4k_policy_evict_first()
@@ -96,11 +103,17 @@ __device__ __forceinline__ unsigned long long t4k_policy_evict_first()
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-// W_4096^t for any t in [0, 4096) from the first quadrant table: W^{t+1024} = -i W^t.
-template <typename T2>
+// W_N^t, N = 1024 TW, for any t in [0, N) from the table of the first 1024 entries: W_4096^{t+1024} = -i W_4096^t,
+// W_2048^{t+1024} = -W_2048^t.
+template <int TW, typename T2>
 __device__ __forceinline__ T2 w4096(const T2 *TQ, int t)
 {
     const T2 w = TQ[t & 1023];
+    if constexpr (TW == 2) {
+        T2 r2 = w;
+        if ((t >> 10) & 1) { r2.x = -w.x; r2.y = -w.y; }
+        return r2;
+    }
     const int quad = (t >> 10) & 3;
     T2 r;
     r.x = (quad & 1) ? w.y : w.x;       // quad 1: -i w = (w.y, -w.x); quad 2: -w; quad 3: i w = (-w.y, w.x)
@@ -164,58 +177,64 @@ __device__ __forceinline__ void fft1024_d(T (&P)[32], T (&Q)[32], T *X, const T2
     }
 }
 
-template <typename T, int RLO, int RHI, bool HAS_EF, int kTeams>
-__global__ void __launch_bounds__(kTeams *kTeamThreads, 1)
+template <typename T, int TW, int RLO, int RHI, bool HAS_EF, int kTeams>
+__global__ void __launch_bounds__(kTeams *TW * 32, 1)
 unfold_t4k_kernel(T4kParams<T> p)
 {
     using T2 = typename T4k<T>::T2;
     using K = T4k<T>;
-    constexpr int kRows = RHI - RLO + 1;            // band rows per thread
-    static_assert(kRows >= 1 && kRows <= 16, "band rows of 128 bins below N/2");
+    static_assert(TW == 1 || TW == 2 || TW == 4, "team of 1, 2 or 4 warps");
+    static_assert(kTeams * TW <= 16 && (TW == 1 || kTeams <= 15), "tensor-memory column blocks / named barriers");
+    constexpr int N = 1024 * TW;
+    constexpr int MPW = 32 / TW;                    // values of m per thread in the radix-TW step
+    constexpr int kRegionX = TW * kPlaneBytes;
+    constexpr int kRows = RHI - RLO + 1;            // band rows per thread (a row = 32 TW bins)
+    static_assert(kRows >= 1 && kRows <= 16, "band rows below N/2");
     constexpr int kMirLo = 31 - RHI, kMirHi = (32 - RLO) > 31 ? 31 : (32 - RLO); // rows holding some band bin's mirror
     constexpr int kMirRows = kMirHi - kMirLo + 1;
-    static_assert(4 * kMirRows * 512 <= kRegionX, "mirror rows fit region X");
+    static_assert(kMirRows * 512 <= kPlaneBytes, "mirror rows fit region X");
     extern __shared__ __align__(128) unsigned char smem[];
-    T2 *TW = reinterpret_cast<T2 *>(smem);        // [32][32] pass twiddles W_1024^{k1 t}
-    T2 *TQ = TW + 1024;                                 // W_4096^t, t < 1024
+    T2 *TW_ = reinterpret_cast<T2 *>(smem);       // [32][32] pass twiddles W_1024^{k1 t}
+    T2 *TQ = TW_ + 1024;                                // W_N^t, t < 1024
     uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabF64);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
-    const int team = warp >> 2, w = warp & 3;
+    const int team = warp / TW, w = warp % TW;
     T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + team * 4;   // [team][4]
-    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + kTeams * 32) + team * 4;
-    unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kTeamBytes;
+    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + 16 * 32) + team * 4;
+    unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kRegionX;
     T *RX = reinterpret_cast<T *>(tb);            // region X
     T *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
 
     if (warp == 0) tmem_alloc_all(tmem_base);
     for (int i = threadIdx.x; i < 1024; i += blockDim.x) {
         const int k1 = i >> 5, t = i & 31;
-        TW[i] = p.tw1024[(k1 * t) & 1023];
+        TW_[i] = p.tw1024[(k1 * t) & 1023];
         TQ[i] = p.twN[i];
     }
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
-    const uint32_t tenv = tmem_addr(*tmem_base, warp, team * 128); // |z_theta|^2: 2 columns per sample, 64 columns
+    const uint32_t tenv = tmem_addr(*tmem_base, warp, (warp >> 2) * 128); // |z_theta|^2: 2 columns per sample, 64 columns
     const uint32_t tephi = tenv + 64;                               // E_phi: 4 columns per band row
 
     const unsigned long long pol_first = t4k_policy_evict_first();
     const long u0 = p.n_units * (long)blockIdx.x / (long)gridDim.x;
     const long u1 = p.n_units * ((long)blockIdx.x + 1) / (long)gridDim.x;
-    constexpr int N = 4096;
 
 #pragma unroll 1
     for (long u = u0 + team; u < u1; u += kTeams) {
         const T *v = p.traces + (size_t)u * 2 * N;
         T *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
         const long ev = u / p.n_stations;
-        const T2 *M = p.minv + (size_t)ev * minv_q4_stride(p.k_lo, p.k_hi) +
+        const int C = (p.k_hi / TW) - (p.k_lo / TW) + 1;         // Minv columns per (q, entry) plane
+        const T2 *M = p.minv + (size_t)ev * 4 * TW * C +
                            (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
         if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(T));
 
         T P[32], Q[32];
-        // ---- a1 + radix-4 step: thread holds y_q[m], q = 0..3, m = lane + 32 (8 w + jj), at [8 q + jj]
+        // ---- a1 + radix-TW step: thread holds y_q[m], q = 0..TW-1, m = lane + 32 (MPW w + jj), at [MPW q + jj]
+        if constexpr (TW == 4) {
         static_for<0, 8>([&](auto jc) {
             constexpr int jj = decltype(jc)::value;
             const int m = lane + 32 * (8 * w + jj);
@@ -238,35 +257,54 @@ unfold_t4k_kernel(T4kParams<T> p)
             t = y2r * w2.x; P[16 + jj] = fma(y2i, -w2.y, t); t = y2r * w2.y; Q[16 + jj] = fma(y2i, w2.x, t);
             t = y3r * w3.x; P[24 + jj] = fma(y3i, -w3.y, t); t = y3r * w3.y; Q[24 + jj] = fma(y3i, w3.x, t);
         });
+        } else if constexpr (TW == 2) {
+        static_for<0, 16>([&](auto jc) {
+            constexpr int jj = decltype(jc)::value;
+            const int m = lane + 32 * (16 * w + jj);
+            const T x0r = K::ld_stream(v + m), x1r = K::ld_stream(v + m + 1024);
+            const T x0i = K::ld_stream(v + N + m), x1i = K::ld_stream(v + N + m + 1024);
+            P[jj] = x0r + x1r; Q[jj] = x0i + x1i;               // y0
+            const T y1r = x0r - x1r, y1i = x0i - x1i;
+            const T2 w1 = TQ[m];                            // W_2048^m, m < 1024
+            T t;
+            t = y1r * w1.x; P[16 + jj] = fma(y1i, -w1.y, t); t = y1r * w1.y; Q[16 + jj] = fma(y1i, w1.x, t);
+        });
+        } else {   // one warp holds the whole station: straight into FFT input order, no exchange
+        static_for<0, 32>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            P[brev5(j)] = K::ld_stream(v + lane + 32 * j);
+            Q[brev5(j)] = K::ld_stream(v + N + lane + 32 * j);
+        });
+        }
 
         // ---- team exchange: warp q collects y_q[lane + 32 j], j = 8 w' + jj, into FFT input order
-        team_sync(team);                                         // region X free (previous station done)
-        {
+        team_sync<TW>(team);                                         // region X free (previous station done)
+        if constexpr (TW > 1) {
             T *XB = RX;                                     // [q][j][lane]
             static_for<0, 32>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;           // i = 8 q + jj
-                XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane] = P[i];
+                constexpr int i = decltype(ic)::value;           // i = MPW q + jj
+                XB[((i / MPW) * 32 + MPW * w + (i % MPW)) * 32 + lane] = P[i];
             });
-            team_sync(team);
+            team_sync<TW>(team);
             static_for<0, 32>([&](auto jc) {
                 constexpr int j = decltype(jc)::value;
                 P[brev5(j)] = XB[(w * 32 + j) * 32 + lane];
             });
-            team_sync(team);
+            team_sync<TW>(team);
             static_for<0, 32>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane] = Q[i];
+                XB[((i / MPW) * 32 + MPW * w + (i % MPW)) * 32 + lane] = Q[i];
             });
-            team_sync(team);
+            team_sync<TW>(team);
             static_for<0, 32>([&](auto jc) {
                 constexpr int j = decltype(jc)::value;
                 Q[brev5(j)] = XB[(w * 32 + j) * 32 + lane];
             });
-            team_sync(team);
+            team_sync<TW>(team);
         }
-        // ---- a2: warp q = w: G[4 (lane + 32 row) + q] in (P[row], Q[row])
-        fft1024_d(P, Q, XW, TW, lane);
-        team_sync(team);                                         // all transposes done: region X becomes the mirror rows
+        // ---- a2: warp q = w: G[TW (lane + 32 row) + q] in (P[row], Q[row])
+        fft1024_d(P, Q, XW, TW_, lane);
+        team_sync<TW>(team);                                         // all transposes done: region X becomes the mirror rows
         {
             T2 *PUB = reinterpret_cast<T2 *>(RX);      // [warp][mirror row][lane]
             static_for<kMirLo, kMirHi + 1>([&](auto rc) {
@@ -274,25 +312,24 @@ unfold_t4k_kernel(T4kParams<T> p)
                 PUB[(w * kMirRows + (r - kMirLo)) * 32 + lane] = K::make2(P[r], Q[r]);
             });
         }
-        team_sync(team);
+        team_sync<TW>(team);
         // ---- separation + a4 on the band rows: E for this warp's bins k = 4 (lane + 32 r) + w, in registers
         T Etr[kRows], Eti[kRows];
         {
             const T2 *PUB = reinterpret_cast<const T2 *>(RX);
-            const int pw = (4 - w) & 3;
+            const int pw = (TW - w) & (TW - 1);
             const int plane = (w == 0) ? ((32 - lane) & 31) : (31 - lane);
             const int padd = (w == 0 && lane == 0) ? 1 : 0;      // q = 0, lane 0: mirror row 32 - r
-            const int C = (p.k_hi >> 2) - (p.k_lo >> 2) + 1;     // Minv columns per (q, entry) plane
             const T2 *Mq = M + (size_t)w * 4 * C;
             static_for<0, kRows>([&](auto rc) {
                 constexpr int i = decltype(rc)::value;
                 constexpr int r = RLO + i;
-                const int k = 4 * (lane + 32 * r) + w;
+                const int k = TW * (lane + 32 * r) + w;
                 const bool inband = k >= p.k_lo && k <= p.k_hi;
                 int prow = 31 - r + padd;
                 prow = prow > kMirHi ? kMirHi : prow;
                 const T2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
-                int c = lane + 32 * r - (p.k_lo >> 2);
+                int c = lane + 32 * r - (p.k_lo / TW);
                 c = c < 0 ? 0 : (c > C - 1 ? C - 1 : c);
                 const T2 m0 = K::ld_nc2(Mq + c), m1 = K::ld_nc2(Mq + C + c);
                 const T2 m2 = K::ld_nc2(Mq + 2 * C + c), m3 = K::ld_nc2(Mq + 3 * C + c);
@@ -308,7 +345,7 @@ unfold_t4k_kernel(T4kParams<T> p)
                 tmem_st64(tephi + 4 * i + 2, K::bits(inband ? fi : (T)0));
             });
         }
-        team_sync(team);                                         // mirror rows consumed: region X is free for transposes
+        team_sync<TW>(team);                                         // mirror rows consumed: region X is free for transposes
 
         // ---- a5/a6: per polarisation, mirror image of the forward path. Warp q inverse-transforms its own
         // bins Z[4 k' + q] (zero outside the band rows), multiplies by W_4096^{-m q}, the team exchanges,
@@ -344,11 +381,11 @@ unfold_t4k_kernel(T4kParams<T> p)
                     }
                 });
             }
-            fft1024_d(Q, P, XW, TW, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
+            fft1024_d(Q, P, XW, TW_, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
             if (w != 0) {
                 // u_q[m] conj(W_4096^{q m}), m = lane + 32 b: two interleaved recurrences over b (ratio W^{64 q})
-                const T2 r2 = w4096(TQ, 64 * w);
-                const T2 c0 = w4096(TQ, (w * lane) & 4095), c1 = w4096(TQ, (w * (lane + 32)) & 4095);
+                const T2 r2 = w4096<TW>(TQ, 64 * w);
+                const T2 c0 = w4096<TW>(TQ, (w * lane) & (N - 1)), c1 = w4096<TW>(TQ, (w * (lane + 32)) & (N - 1));
                 T er = c0.x, ei = c0.y, orr = c1.x, oi = c1.y;
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
@@ -364,31 +401,40 @@ unfold_t4k_kernel(T4kParams<T> p)
                     }
                 });
             }
-            team_sync(team);                                     // all transposes done: region X is the exchange buffer
-            {
+            team_sync<TW>(team);                                     // all transposes done: region X is the exchange buffer
+            if constexpr (TW > 1) {
                 T *XB = RX;                                 // [q][b][lane]
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
                     XB[(w * 32 + b) * 32 + lane] = P[b];
                 });
-                team_sync(team);
+                team_sync<TW>(team);
                 static_for<0, 32>([&](auto ic) {
-                    constexpr int i = decltype(ic)::value;       // i = 8 q + jj
-                    P[i] = XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane];
+                    constexpr int i = decltype(ic)::value;       // i = MPW q + jj
+                    P[i] = XB[((i / MPW) * 32 + MPW * w + (i % MPW)) * 32 + lane];
                 });
-                team_sync(team);
+                team_sync<TW>(team);
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
                     XB[(w * 32 + b) * 32 + lane] = Q[b];
                 });
-                team_sync(team);
+                team_sync<TW>(team);
                 static_for<0, 32>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    Q[i] = XB[((i >> 3) * 32 + 8 * w + (i & 7)) * 32 + lane];
+                    Q[i] = XB[((i / MPW) * 32 + MPW * w + (i % MPW)) * 32 + lane];
                 });
-                team_sync(team);
+                team_sync<TW>(team);
             }
-            // radix-4 step (inverse sign): z_s = sum_q (+i)^{s q} u_q, left in place at [8 s + jj]
+            // radix-TW step (inverse sign): z_s = sum_q (+i)^{s q} u_q (TW = 4), left in place at [MPW s + jj]
+            if constexpr (TW == 2) {
+                static_for<0, 16>([&](auto jc) {
+                    constexpr int jj = decltype(jc)::value;
+                    const T ar = P[jj], ai = Q[jj];
+                    P[jj] = ar + P[16 + jj]; Q[jj] = ai + Q[16 + jj];
+                    P[16 + jj] = ar - P[16 + jj]; Q[16 + jj] = ai - Q[16 + jj];
+                });
+            }
+            if constexpr (TW == 4)
             static_for<0, 8>([&](auto jc) {
                 constexpr int jj = decltype(jc)::value;
                 const T ar = P[jj] + P[16 + jj], ai = Q[jj] + Q[16 + jj];
@@ -400,12 +446,12 @@ unfold_t4k_kernel(T4kParams<T> p)
                 P[16 + jj] = ar - cr; Q[16 + jj] = ai - ci;
                 P[24 + jj] = br + di; Q[24 + jj] = bi - dr;      // b - i d
             });
-            // outputs: index i = 8 s + jj is sample n = lane + 32 (8 w + jj) + 1024 s (ascending in i)
-            const int nbase = lane + 256 * w;
+            // outputs: index i = MPW s + jj is sample n = lane + 32 (MPW w + jj) + 1024 s (ascending in i)
+            const int nbase = lane + 32 * MPW * w;
             if (pol == 0) {
                 static_for<0, 32>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    if (HAS_EF) K::st_stream(ef + nbase + 32 * (i & 7) + 1024 * (i >> 3), P[i], pol_first);
+                    if (HAS_EF) K::st_stream(ef + nbase + 32 * (i % MPW) + 1024 * (i / MPW), P[i], pol_first);
                     T e2 = P[i] * P[i]; e2 = fma(Q[i], Q[i], e2);
                     tmem_st64(tenv + 2 * i, K::bits(e2));
                 });
@@ -426,7 +472,7 @@ unfold_t4k_kernel(T4kParams<T> p)
                     static_for<0, 8>([&](auto jc) {
                         constexpr int j = decltype(jc)::value;
                         constexpr int i = 8 * c + j;
-                        const int n = nbase + 32 * (i & 7) + 1024 * (i >> 3);
+                        const int n = nbase + 32 * (i % MPW) + 1024 * (i / MPW);
                         if (HAS_EF) K::st_stream(ef + N + n, P[i], pol_first);
                         T e2 = fma(P[i], P[i], K::from_bits(ev[j]));
                         e2 = fma(Q[i], Q[i], e2);
@@ -443,12 +489,16 @@ unfold_t4k_kernel(T4kParams<T> p)
             const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
             if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
         }
+        if constexpr (TW == 1) {
+            if (lane == 0) { p.amp[u] = sqrt(best); p.idx[u] = bi; }
+            continue;
+        }
         if (lane == 0) { peak_v[w] = best; peak_i[w] = bi; }
-        team_sync(team);
+        team_sync<TW>(team);
         if (w == 0 && lane == 0) {
             T bv = peak_v[0]; int bx = peak_i[0];
 #pragma unroll
-            for (int i = 1; i < 4; ++i)
+            for (int i = 1; i < TW; ++i)
                 if (peak_v[i] > bv || (peak_v[i] == bv && peak_i[i] < bx)) { bv = peak_v[i]; bx = peak_i[i]; }
             p.amp[u] = sqrt(bv); p.idx[u] = bx;
         }
@@ -458,16 +508,16 @@ unfold_t4k_kernel(T4kParams<T> p)
     if (warp == 0) tmem_free_all(*tmem_base);
 }
 
-template <typename T, int RLO, int RHI, bool HAS_EF>
+template <typename T, int TW, int RLO, int RHI, bool HAS_EF>
 cudaError_t launch_t4k(const T4kParams<T> &q, cudaStream_t s)
 {
-    constexpr int kTeams = kTeamsOf<T>;
-    const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * kTeamBytes;
-    auto kern = unfold_t4k_kernel<T, RLO, RHI, HAS_EF, kTeams>;
+    constexpr int kTeams = kTeamsOf<T> * 4 / TW;       // the same warps per CTA for every team size
+    const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * TW * kPlaneBytes;
+    auto kern = unfold_t4k_kernel<T, TW, RLO, RHI, HAS_EF, kTeams>;
     AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + kTeams - 1) / kTeams;
     if (grid > sm_count()) grid = sm_count();
-    kern<<<(unsigned)grid, kTeams * kTeamThreads, smem, s>>>(q);
+    kern<<<(unsigned)grid, kTeams * TW * 32, smem, s>>>(q);
     return cudaGetLastError();
 }
 
@@ -481,17 +531,26 @@ cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, con
     q.minv = (const T2 *)minv; q.tw1024 = (const T2 *)p.tw1024; q.twN = (const T2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
+    if (p.N == 1024) return efield ? launch_t4k<T, 1, 0, 15, true>(q, s) : launch_t4k<T, 1, 0, 15, false>(q, s);
+    if constexpr (sizeof(T) == 8) {     // (fp32 N = 2048 is the warp kernel's)
+        if (p.N == 2048) return efield ? launch_t4k<T, 2, 0, 15, true>(q, s) : launch_t4k<T, 2, 0, 15, false>(q, s);
+    }
     // rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3]) have their own instantiation; <0, 15> serves any other band
-    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) return efield ? launch_t4k<T, 4, 12, true>(q, s) : launch_t4k<T, 4, 12, false>(q, s);
-    return efield ? launch_t4k<T, 0, 15, true>(q, s) : launch_t4k<T, 0, 15, false>(q, s);
+    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) return efield ? launch_t4k<T, 4, 4, 12, true>(q, s) : launch_t4k<T, 4, 4, 12, false>(q, s);
+    return efield ? launch_t4k<T, 4, 0, 15, true>(q, s) : launch_t4k<T, 4, 0, 15, false>(q, s);
 }
 
 } // namespace
 
-bool t4k_supported(int dtype, const PlanDev &p)
+int t4k_team_warps(int dtype, const PlanDev &p)
 {
-    return (dtype == AERA_F64 || dtype == AERA_F32) && p.N == 4096 && p.k_lo >= 1 && p.k_hi < 2048;
+    if (p.k_lo < 1 || p.k_hi >= p.N / 2) return 0;
+    if (p.N == 4096 && (dtype == AERA_F64 || dtype == AERA_F32)) return 4;
+    if (p.N == 2048 && dtype == AERA_F64) return 2;
+    if (p.N == 1024 && (dtype == AERA_F64 || dtype == AERA_F32)) return 1;
+    return 0;
 }
+bool t4k_supported(int dtype, const PlanDev &p) { return t4k_team_warps(dtype, p) != 0; }
 
 cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                               void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x)

@@ -95,7 +95,7 @@ __device__ __forceinline__ void separate_solve(const R *QA, const R *QB, const f
         // loads of neighbouring rows are independent and the unrolled iterations overlap their latencies
         // rows of a band-specific instantiation reach at most 31 bins beyond the band: Minv is zero-padded there
         // (MINV_PACKED_PAD), so E = 0 comes out of the arithmetic; the any-band instantiation clamps and selects
-        constexpr bool kAnyBand = G::kLo == 0 && G::kHi == 31;
+        constexpr bool kAnyBand = !G::kExact;   // instantiation rows are a superset of the band's rows
         const bool inband = !kAnyBand || (k >= k_lo && k <= k_hi);
         int j = k - k_lo;
         if (kAnyBand) j = j < 0 ? 0 : (j > k_hi - k_lo ? k_hi - k_lo : j);
@@ -406,12 +406,36 @@ bool w32_supported(int dtype, const PlanDev &p)
     return dtype == AERA_F32 && p.N == 2 * kM && p.k_hi < kM && p.k_lo >= 1;
 }
 
+// Row geometries instantiated: <10, 28> exactly configs[1]'s rows (30-80 MHz at fs = 180 MHz); <6, 28> any band inside
+// bins 192..927 (30-80 MHz at sampling rates of 180-250 MHz: still twelve warps and the per-event Minv ring);
+// <0, 31> everything else (eight warps, Minv through L1/L2).
+static int w32_geom(const PlanDev &p)
+{
+    const int lo = p.k_lo >> 5, hi = p.k_hi >> 5;
+    if (lo == 10 && hi == 28) return 0;
+    if (lo >= 6 && hi <= 28) return 1;
+    return 2;
+}
+
 size_t w32_spectra_bytes(const PlanDev &p, long n_units)
 {
-    // rows 10..28 (configs[1]) store their 19 band rows, any other band all 32 rows
-    const int rows = ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) ? W32Geom<10, 28>::kBandRows : 32;
+    const int g = w32_geom(p);
+    const int rows = g == 0 ? W32Geom<10, 28>::kBandRows : (g == 1 ? W32Geom<6, 28>::kBandRows : 32);
     return (size_t)n_units * rows * 32 * sizeof(float4);
 }
+
+namespace {
+// MINV_RING: the geometry stages Minv per event in shared memory (unless several tables are resident)
+template <int K2LO, int K2HI, bool MINV_RING>
+cudaError_t launch_geom(const W32Params &q, cudaStream_t s, bool ef, bool i16, bool multi, int spec)
+{
+    if (i16) return ef ? launch_inst<K2LO, K2HI, true, MINV_RING, 0, true>(q, s) : launch_inst<K2LO, K2HI, false, MINV_RING, 0, true>(q, s);
+    if (multi) return ef ? launch_inst<K2LO, K2HI, true, false, 0>(q, s) : launch_inst<K2LO, K2HI, false, false, 0>(q, s);
+    if (spec == 1) return ef ? launch_inst<K2LO, K2HI, true, MINV_RING, 1>(q, s) : launch_inst<K2LO, K2HI, false, MINV_RING, 1>(q, s);
+    if (spec == 2) return ef ? launch_inst<K2LO, K2HI, true, MINV_RING, 2>(q, s) : launch_inst<K2LO, K2HI, false, MINV_RING, 2>(q, s);
+    return ef ? launch_inst<K2LO, K2HI, true, MINV_RING, 0>(q, s) : launch_inst<K2LO, K2HI, false, MINV_RING, 0>(q, s);
+}
+} // namespace
 
 cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                               void *amp, int32_t *idx, const void *minv, cudaStream_t s, void *spectra, int spec_mode,
@@ -426,24 +450,14 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
     q.spectra = (float4 *)spectra;
     q.minv = (const float4 *)minv; q.tw1024 = (const float2 *)p.tw1024; q.twN = (const float2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
+    const int spec = spectra ? spec_mode : 0;
+    const bool ef = efield != nullptr, i16 = x.input_i16 != 0, multi = x.pattern_id != nullptr;
     cudaError_t e;
-    const bool cfg1_rows = (p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28;   // configs[1]: 30-80 MHz at fs = 180 MHz
-    if (x.input_i16) {           // int16 ADC counts in (Minv staged per event; one table)
-        if (cfg1_rows) e = efield ? launch_inst<10, 28, true, true, 0, true>(q, s) : launch_inst<10, 28, false, true, 0, true>(q, s);
-        else e = efield ? launch_inst<0, 31, true, false, 0, true>(q, s) : launch_inst<0, 31, false, false, 0, true>(q, s);
-    } else if (x.pattern_id) {   // one Minv per (event, antenna type): read through L1/L2 instead of the per-event smem ring
-        if (cfg1_rows) e = efield ? launch_inst<10, 28, true, false, 0>(q, s) : launch_inst<10, 28, false, false, 0>(q, s);
-        else e = efield ? launch_inst<0, 31, true, false, 0>(q, s) : launch_inst<0, 31, false, false, 0>(q, s);
-    } else if (cfg1_rows) {
-        if (spectra && spec_mode == 1) e = efield ? launch_inst<10, 28, true, true, 1>(q, s) : launch_inst<10, 28, false, true, 1>(q, s);
-        else if (spectra && spec_mode == 2) e = efield ? launch_inst<10, 28, true, true, 2>(q, s) : launch_inst<10, 28, false, true, 2>(q, s);
-        else e = efield ? launch_inst<10, 28, true, true, 0>(q, s) : launch_inst<10, 28, false, true, 0>(q, s);
-    } else if (spectra && spec_mode == 1)
-        e = efield ? launch_inst<0, 31, true, false, 1>(q, s) : launch_inst<0, 31, false, false, 1>(q, s);
-    else if (spectra && spec_mode == 2)
-        e = efield ? launch_inst<0, 31, true, false, 2>(q, s) : launch_inst<0, 31, false, false, 2>(q, s);
-    else
-        e = efield ? launch_inst<0, 31, true, false, 0>(q, s) : launch_inst<0, 31, false, false, 0>(q, s);
+    switch (w32_geom(p)) {
+    case 0: e = launch_geom<10, 28, true>(q, s, ef, i16, multi, spec); break;
+    case 1: e = launch_geom<6, 28, true>(q, s, ef, i16, multi, spec); break;
+    default: e = launch_geom<0, 31, false>(q, s, ef, i16, multi, spec); break;
+    }
     count_launches(1);
     return e;
 }

@@ -261,6 +261,9 @@ __device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], i
 template <int K2LO, int K2HI>
 struct W32Geom {
     static constexpr int kLo = K2LO, kHi = K2HI;
+    // <10, 28> is used only for bands whose rows are exactly 10..28 (configs[1]); every other geometry serves any band
+    // whose rows lie inside it, so its edge rows may be entirely out of band
+    static constexpr bool kExact = K2LO == 10 && K2HI == 28;
     static constexpr int kBandRows = K2HI - K2LO + 1;
     // rows that hold some band bin's mirror 1024-k: row 31-r for lanes >= 1, row 32-r for lane 0
     static constexpr int kMirLo = 31 - K2HI;

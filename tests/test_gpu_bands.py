@@ -20,11 +20,14 @@ def B():
 @pytest.mark.parametrize("dtype,N,fs,kernel", [("f32", 2048, 200e6, "unfold_w32"), ("f32", 2048, 250e6, "unfold_w32"),
                                                ("f64", 4096, 250e6, "unfold_t4k_f64"), ("f64", 4096, 180e6, "unfold_t4k_f64"),
                                                ("f32", 4096, 200e6, "unfold_t4k_f32"), ("f32", 4096, 250e6, "unfold_t4k_f32"),
-                                               ("f32", 1024, 200e6, "generic"), ("f64", 2048, 200e6, "generic")])
+                                               ("f32", 1024, 200e6, "unfold_t1k_f32"), ("f32", 1024, 180e6, "unfold_t1k_f32"),
+                                               ("f64", 2048, 200e6, "unfold_t2k_f64"), ("f64", 2048, 250e6, "unfold_t2k_f64"),
+                                               ("f64", 1024, 200e6, "unfold_t1k_f64"), ("f64", 1024, 180e6, "unfold_t1k_f64"),
+                                               ("f32", 512, 200e6, "generic"), ("f64", 8192, 200e6, "generic")])
 def test_batch_other_bands(B, dtype, N, fs, kernel):
     import oracle
     base = ai.WORKLOADS[0]
-    wl = ai.Workload(91, "bands", 3, 6, N, fs, dtype, base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
+    wl = ai.Workload(91, "bands", 3, 7, N, fs, dtype, base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
     H = ai.pattern_table(wl.grid, wl.complex_dtype)
     tr, dirs, _, _ = ai.make_batch(wl, range(3))
     dt = B.AERA_F32 if dtype == "f32" else B.AERA_F64
