@@ -113,7 +113,7 @@ struct ScanGeom {
     static constexpr int kWarps = kScanStations * kDirs;         // 12 (three warps per scheduler) or 8
     static constexpr int kColStride = 512 / kDirs;
     static_assert(kCols <= kColStride, "tensor-memory columns per warp");
-    static constexpr bool kAnyBand = K2LO == 0 && K2HI == 31;    // rows may lie wholly outside the band: clamp every Minv index
+    static constexpr bool kAnyBand = !G::kExact;                 // rows may lie wholly outside the band: clamp every Minv index
 };
 
 template <int K2LO, int K2HI>
@@ -295,7 +295,7 @@ scan_inv_w32_kernel(ScanParams p)
 
 bool scan_w32_supported(int dtype, const PlanDev &p)
 {
-    // rows 10..28 (30-80 MHz at fs = 180 MHz, configs[2]) have their own instantiation; <0, 31> serves any other band
+    // rows 10..28 (30-80 MHz at fs = 180 MHz, configs[2]) have their own instantiation; <7, 27> and <0, 31> serve the other bands
     return dtype == AERA_F32 && p.N == 2 * kM && p.k_hi < kM && p.k_lo >= 1;
 }
 
@@ -337,7 +337,11 @@ cudaError_t launch_scan_w32(const PlanDev &p, int n_stations, const void *traces
     q.traces = (const float *)traces; q.spectra = (float4 *)spectra; q.minv = (const float4 *)minv;
     q.amp = (float *)amp; q.idx = idx; q.tw1024 = (const float2 *)p.tw1024; q.twN = (const float2 *)p.twN;
     q.n_dirs = n_dirs; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
-    const cudaError_t e = ((p.k_lo >> 5) == 10 && (p.k_hi >> 5) == 28) ? launch_scan_inst<10, 28>(q, s) : launch_scan_inst<0, 31>(q, s);
+    // <10, 28>: exactly configs[2]'s rows; <7, 27>: any band inside bins 224..895 (30-80 MHz at fs = 200-250 MHz), 21 rows:
+    // still three directions per tile / twelve warps; <0, 31>: everything else (two directions per tile, eight warps)
+    const int lo = p.k_lo >> 5, hi = p.k_hi >> 5;
+    const cudaError_t e = (lo == 10 && hi == 28) ? launch_scan_inst<10, 28>(q, s)
+                          : ((lo >= 7 && hi <= 27) ? launch_scan_inst<7, 27>(q, s) : launch_scan_inst<0, 31>(q, s));
     count_launches(2);
     return e;
 }
