@@ -43,10 +43,16 @@ constexpr int kLCluster = 8;               // CTAs per station (thread-block clu
 inline int long_max_clusters() { return sm_count() * kLCtasPerSm / kLCluster; }   // 55 stations in flight on 148 SMs
 constexpr int kLTeam = kLWarps * kLCluster;
 constexpr size_t kYBytes = (size_t)32 * 1024 * 16;            // Y[q][mm] two 8-byte planes; reused as U[2][16][1024]
-// band geometry of the one instantiation (configs[4]: k = 1311 .. 13107)
-constexpr int kP2Lo = 1, kP2Hi = 12;      // phase 2 rows (k' >> 5, k' = k >> 5)
-constexpr int kP3Lo = 2, kP3Hi = 25;      // phase 3 rows (k'' >> 5, k'' = k >> 4)
-constexpr int kMirLoL = 31 - kP2Hi, kMirRowsL = 32 - kMirLoL; // mirror rows 19..31 published to the pair partner
+// band geometry of an instantiation: phase 2 rows P2LO..P2HI (k' >> 5, k' = k >> 5, i.e. k >> 10) and phase 3 rows
+// 2 P2LO .. 2 P2HI + 1 (k'' >> 5, k'' = k >> 4, i.e. k >> 9). <1, 12> is configs[4] (k = 1311 .. 13107); <0, 15> serves
+// any other band below N/4.
+template <int P2LO, int P2HI>
+struct LongGeom {
+    static constexpr int kP2Lo = P2LO, kP2Hi = P2HI;
+    static constexpr int kP3Lo = 2 * P2LO, kP3Hi = 2 * P2HI + 1;
+    static constexpr int kMirLoL = 31 - P2HI, kMirRowsL = 32 - kMirLoL;   // mirror rows published to the pair partner
+    static_assert(P2LO >= 0 && P2HI <= 15 && 2 * kMirRowsL * 256 <= kXBytes, "rows below N/4; mirror rows fit the warp buffer");
+};
 
 struct LongParams {
     const float *traces;
@@ -191,10 +197,13 @@ __device__ __forceinline__ void ifft16(R (&xr)[16], R (&xi)[16])
     });
 }
 
-template <bool HAS_EF>
+template <bool HAS_EF, int P2LO, int P2HI>
 __global__ void __cluster_dims__(kLCluster, 1, 1) __launch_bounds__(kLWarps * 32, kLCtasPerSm)
 unfold_long_f32_kernel(LongParams p)
 {
+    using LG = LongGeom<P2LO, P2HI>;
+    constexpr int kP2Lo = LG::kP2Lo, kP2Hi = LG::kP2Hi, kP3Lo = LG::kP3Lo, kP3Hi = LG::kP3Hi;
+    constexpr int kMirLoL = LG::kMirLoL, kMirRowsL = LG::kMirRowsL;
     extern __shared__ __align__(128) unsigned char smem[];
     float2 *T = reinterpret_cast<float2 *>(smem);                       // [32][32] pass twiddles W_1024^{k1 t}
     float2 *TA = T + 1024;                                              // W_N^{256 a}
@@ -296,7 +305,8 @@ unfold_long_f32_kernel(LongParams p)
                 else w = cmulf(w, rat);
                 const int kp = lane + 32 * k2, k = 32 * kp + q;
                 const bool inband = k >= p.k_lo && k <= p.k_hi;
-                const int prow = 31 - k2 + padd - kMirLoL;
+                int prow = 31 - k2 + padd - kMirLoL;
+                if (kP2Lo == 0 && prow > kMirRowsL - 1) prow = kMirRowsL - 1;   // (k = 0, whose mirror row would be 32, is never in band)
                 const R ar = A[k2], ai = B[k2], pr = PUB[prow * 32 + plane], pi = PUB[(kMirRowsL + prow) * 32 + plane];
                 const R f0r = L::add(ar, pr), f0i = L::sub(ai, pi);
                 const R f1r = L::add(ai, pi), f1i = L::sub(pr, ar);
@@ -448,9 +458,9 @@ unfold_long_f32_kernel(LongParams p)
 
 bool long_f32_supported(int dtype, const PlanDev &p)
 {
-    // the one band geometry instantiated (configs[4]: 20-200 MHz at fs = 1 GHz): rows as in kP2*/kP3*
-    return dtype == AERA_F32 && p.N == kLN && p.k_lo >= 1 && p.k_hi < kLN / 4 &&
-           (p.k_lo >> 10) == kP2Lo && (p.k_hi >> 10) == kP2Hi && (p.k_lo >> 9) == kP3Lo && (p.k_hi >> 9) == kP3Hi;
+    // any band below N/4 (the inverse transforms are quarter-pruned); configs[4]'s rows (20-200 MHz at fs = 1 GHz) have
+    // their own instantiation
+    return dtype == AERA_F32 && p.N == kLN && p.k_lo >= 1 && p.k_hi < kLN / 4;
 }
 
 static size_t long_stride(const PlanDev &p)
@@ -494,7 +504,10 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
         kern<<<(unsigned)(kLCluster * clusters), kLWarps * 32, smem, s>>>(q);
         return cudaGetLastError();
     };
-    e = efield ? launch(unfold_long_f32_kernel<true>) : launch(unfold_long_f32_kernel<false>);
+    if ((p.k_lo >> 10) == 1 && (p.k_hi >> 10) == 12)
+        e = efield ? launch(unfold_long_f32_kernel<true, 1, 12>) : launch(unfold_long_f32_kernel<false, 1, 12>);
+    else
+        e = efield ? launch(unfold_long_f32_kernel<true, 0, 15>) : launch(unfold_long_f32_kernel<false, 0, 15>);
     count_launches(1);
     return e;
 }

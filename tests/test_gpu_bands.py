@@ -45,6 +45,29 @@ def test_batch_other_bands(B, dtype, N, fs, kernel):
     assert rep.ok(TOL[dtype]), str(rep)
 
 
+@pytest.mark.parametrize("fs", [1e9, 500e6])
+def test_long_trace_other_band(B, fs):
+    """N = 65536 with the 30-80 MHz table (configs[4]'s is 20-200 MHz): the cluster kernel's any-band instantiation."""
+    import oracle
+    base = ai.WORKLOADS[0]
+    N = 65536
+    wl = ai.Workload(94, "long-band", 1, 3, N, fs, "f32", base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    tr, dirs, _, _ = ai.make_batch(wl, range(1))
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        ef, amp, idx = B.aera_unfold_batch(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(dirs).cuda(), fs)
+        torch.cuda.synchronize()
+        assert B.aera_last_kernel() == "unfold_long_f32"
+    finally:
+        pat.free()
+    E, S = tr.shape[:2]
+    ref = oracle.unfold_batch(wl.grid, H, fs, tr.reshape(E * S, 2, -1), np.repeat(dirs, S, axis=0), want_env2=True)
+    rep = compare("f32", ef.cpu().numpy().reshape(E * S, 2, -1), amp.cpu().numpy().ravel(), idx.cpu().numpy().ravel(), ref)
+    print(f"\n[long trace, 30-80 MHz table, fs={fs / 1e6:.0f} MHz] {rep}")
+    assert rep.ok(TOL["f32"]), str(rep)
+
+
 def test_scan_other_band_runs_the_warp_kernels(B):
     import oracle
     base = ai.WORKLOADS[2]
