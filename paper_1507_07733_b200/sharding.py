@@ -21,6 +21,15 @@ def shard_range(n_items: int, rank: int, world: int) -> range:
     return range(n_items * rank // world, n_items * (rank + 1) // world)
 
 
+def scan_shard(dirs, rank: int, world: int):
+    """`aera_scan_directions` across ranks: rank r scans the contiguous block shard_range(n_dirs, r, world) of the
+    direction list against ALL stations (the forward spectra are recomputed per rank: 124 transforms against
+    ~10^5 pairs). The peaks are [n_dirs][n_stations], direction-major, so the ranks' outputs concatenated in rank
+    order (gather_peaks) are the single-GPU result. The total work is fixed as the ranks grow: strong scaling."""
+    sh = shard_range(int(dirs.shape[0]), rank, world)
+    return dirs[sh.start:sh.stop]
+
+
 def weak_events(n_events_per_gpu: int, rank: int) -> range:
     """Weak scaling (bench.py): every rank processes its own n_events_per_gpu canonical events."""
     return range(rank * n_events_per_gpu, (rank + 1) * n_events_per_gpu)

@@ -32,6 +32,16 @@ def test_weak_events_are_disjoint():
     assert set(a).isdisjoint(b) and len(a) == len(b) == 200 and b[0] == 200
 
 
+def test_scan_shards_reassemble_in_direction_order():
+    import numpy as np
+    import aera_inputs as ai
+    dirs = ai.scan_directions()
+    for world in (1, 2, 3, 8):
+        parts = [sharding.scan_shard(dirs, r, world) for r in range(world)]
+        assert np.array_equal(np.concatenate(parts), dirs)
+        assert max(len(p) for p in parts) - min(len(p) for p in parts) <= 1
+
+
 def test_aggregate_single_process():
     u, ms, v = sharding.aggregate_throughput(124000, 1.0)
     assert (u, ms) == (124000, 1.0) and abs(v - 1.24e8) < 1e-3
