@@ -531,13 +531,20 @@ cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, con
     q.minv = (const T2 *)minv; q.tw1024 = (const T2 *)p.tw1024; q.twN = (const T2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
-    if (p.N == 1024) return efield ? launch_t4k<T, 1, 0, 15, true>(q, s) : launch_t4k<T, 1, 0, 15, false>(q, s);
+    // rows 4..12 of 32 TW bins (30-80 MHz at fs = 200 MHz for every N; configs[3]) have their own instantiation; <0, 15> serves
+    // any other band
+    const int tw = p.N / 1024;
+    const bool r412 = (p.k_lo / (32 * tw)) == 4 && (p.k_hi / (32 * tw)) == 12;
+    auto pick = [&](auto twc) -> cudaError_t {
+        constexpr int TWc = decltype(twc)::value;
+        if (r412) return efield ? launch_t4k<T, TWc, 4, 12, true>(q, s) : launch_t4k<T, TWc, 4, 12, false>(q, s);
+        return efield ? launch_t4k<T, TWc, 0, 15, true>(q, s) : launch_t4k<T, TWc, 0, 15, false>(q, s);
+    };
+    if (tw == 1) return pick(IC<1>{});
     if constexpr (sizeof(T) == 8) {     // (fp32 N = 2048 is the warp kernel's)
-        if (p.N == 2048) return efield ? launch_t4k<T, 2, 0, 15, true>(q, s) : launch_t4k<T, 2, 0, 15, false>(q, s);
+        if (tw == 2) return pick(IC<2>{});
     }
-    // rows 4..12 of 128 bins (30-80 MHz at fs = 200 MHz, configs[3]) have their own instantiation; <0, 15> serves any other band
-    if ((p.k_lo >> 7) == 4 && (p.k_hi >> 7) == 12) return efield ? launch_t4k<T, 4, 4, 12, true>(q, s) : launch_t4k<T, 4, 4, 12, false>(q, s);
-    return efield ? launch_t4k<T, 4, 0, 15, true>(q, s) : launch_t4k<T, 4, 0, 15, false>(q, s);
+    return pick(IC<4>{});
 }
 
 } // namespace
