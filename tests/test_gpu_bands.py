@@ -109,3 +109,53 @@ def test_spectrum_reuse_on_another_band_is_bit_identical(B):
             assert torch.equal(a[k], b[k]), k
     finally:
         pat.free()
+
+
+@pytest.mark.parametrize("dtype,N,kernel", [("f64", 1024, "unfold_t1k_f64"), ("f64", 2048, "unfold_t2k_f64"), ("f32", 1024, "unfold_t1k_f32")])
+def test_team_sizes_fold_inplace_peaks_only_and_tables(B, dtype, N, kernel):
+    """Teams of one and two warps (N = 1024 / 2048) through every entry point that shares the team kernel: the forward
+    model against the oracle's fold, E-field written over the traces, peaks only, and two identical tables reproducing
+    the single-table call bit for bit; 3 x 7 = 21 stations do not fill the CTA's teams evenly."""
+    import oracle
+    base = ai.WORKLOADS[0]
+    fs = 200e6
+    wl = ai.Workload(95, "team-sizes", 3, 7, N, fs, dtype, base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    tr, dirs, _, _ = ai.make_batch(wl, range(3))
+    dt = B.AERA_F32 if dtype == "f32" else B.AERA_F64
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    pat2 = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    try:
+        d_tr = torch.from_numpy(tr).cuda(); d_dirs = torch.from_numpy(dirs).cuda()
+        ef, amp, idx = B.aera_unfold_batch(pat, d_tr, d_dirs, fs)
+        assert B.aera_last_kernel() == kernel
+        # peaks only
+        _, amp1, idx1 = B.aera_unfold_batch(pat, d_tr, d_dirs, fs, want_efield=False)
+        assert torch.equal(amp, amp1) and torch.equal(idx, idx1)
+        # two identical tables, stations alternating between them
+        pid = torch.tensor([s & 1 for s in range(7)], dtype=torch.int32, device="cuda")
+        ef2, amp2, idx2 = B.aera_unfold_batch_multi([pat, pat2], pid, d_tr, d_dirs, fs)
+        assert B.aera_last_kernel() == kernel
+        assert torch.equal(ef, ef2) and torch.equal(amp, amp2) and torch.equal(idx, idx2)
+        # in place
+        d_io = d_tr.clone()
+        ef3, amp3, idx3 = B.aera_unfold_batch(pat, d_io, d_dirs, fs, efield=d_io)
+        assert torch.equal(ef, ef3) and torch.equal(amp, amp3) and torch.equal(idx, idx3)
+        # forward model on the same kernels
+        rng = np.random.default_rng([78, N])
+        e_in = rng.standard_normal((2, 5, 2, N)).astype(wl.real_dtype)
+        v = B.aera_fold_batch(pat, torch.from_numpy(e_in).cuda(), d_dirs[:2].contiguous(), fs)
+        assert B.aera_last_kernel() == kernel
+        torch.cuda.synchronize()
+        v_h = v.cpu().numpy()
+    finally:
+        pat.free(); pat2.free()
+    k_lo, k_hi = oracle.band(N, fs, wl.grid.n_freq, wl.grid.freq0_hz, wl.grid.dfreq_hz)
+    worst = 0.0
+    for e in range(2):
+        for s in range(5):
+            Et = oracle.dft_band(e_in[e, s, 0], k_lo, k_hi); Ep = oracle.dft_band(e_in[e, s, 1], k_lo, k_hi)
+            ref = oracle.fold_station(wl.grid, H, N, fs, Et, Ep, dirs[e, 0], dirs[e, 1])
+            worst = max(worst, np.linalg.norm(v_h[e, s] - ref) / np.linalg.norm(ref))
+    print(f"\n[team sizes {dtype} N={N}] fold max rel L2 vs oracle = {worst:.3e}")
+    assert worst <= TOL[dtype]["l2"], worst
