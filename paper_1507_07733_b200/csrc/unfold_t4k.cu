@@ -71,7 +71,7 @@ template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? AERA_T4K_TEAMS_F
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane (sized for fp64)
 // region X of a team = TW planes (33 792 B at TW = 4): exchange buffer / transpose planes / mirror rows
 constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_N^t, t < 1024)
-constexpr int kCtlF64 = 1024;                         // TMEM base, per-team peak slots (up to 16 teams)
+constexpr int kCtlF64 = 512;                          // TMEM base, per-team peak slots (teams of 2 or 4 warps: at most 8 teams)
 
 template <typename T>
 struct T4kParams {
@@ -199,9 +199,10 @@ unfold_t4k_kernel(T4kParams<T> p)
     uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabF64);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
-    const int team = warp / TW, w = warp % TW;
-    T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + team * 4;   // [team][4]
-    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + 16 * 32) + team * 4;
+    constexpr int kLogTW = TW == 4 ? 2 : (TW == 2 ? 1 : 0);
+    const int team = warp >> kLogTW, w = warp & (TW - 1);   // (shifts and masks: a signed division hides w's range from the compiler)
+    T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + (TW == 1 ? 0 : team) * 4;   // [team][4]
+    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + (TW == 1 ? 0 : kTeams) * 32) + team * 4;   // (unused when TW = 1)
     unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kRegionX;
     T *RX = reinterpret_cast<T *>(tb);            // region X
     T *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
@@ -227,8 +228,7 @@ unfold_t4k_kernel(T4kParams<T> p)
         const T *v = p.traces + (size_t)u * 2 * N;
         T *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
         const long ev = u / p.n_stations;
-        const int C = (p.k_hi / TW) - (p.k_lo / TW) + 1;         // Minv columns per (q, entry) plane
-        const T2 *M = p.minv + (size_t)ev * 4 * TW * C +
+        const T2 *M = p.minv + (size_t)ev * ((size_t)(4 * TW) * ((p.k_hi >> kLogTW) - (p.k_lo >> kLogTW) + 1)) +
                            (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
         if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(T));
 
@@ -317,6 +317,7 @@ unfold_t4k_kernel(T4kParams<T> p)
         T Etr[kRows], Eti[kRows];
         {
             const T2 *PUB = reinterpret_cast<const T2 *>(RX);
+            const int C = (p.k_hi >> kLogTW) - (p.k_lo >> kLogTW) + 1;     // Minv columns per (q, entry) plane
             const int pw = (TW - w) & (TW - 1);
             const int plane = (w == 0) ? ((32 - lane) & 31) : (31 - lane);
             const int padd = (w == 0 && lane == 0) ? 1 : 0;      // q = 0, lane 0: mirror row 32 - r
@@ -329,7 +330,7 @@ unfold_t4k_kernel(T4kParams<T> p)
                 int prow = 31 - r + padd;
                 prow = prow > kMirHi ? kMirHi : prow;
                 const T2 gm = PUB[(pw * kMirRows + (prow - kMirLo)) * 32 + plane];
-                int c = lane + 32 * r - (p.k_lo / TW);
+                int c = lane + 32 * r - (p.k_lo >> kLogTW);
                 c = c < 0 ? 0 : (c > C - 1 ? C - 1 : c);
                 const T2 m0 = K::ld_nc2(Mq + c), m1 = K::ld_nc2(Mq + C + c);
                 const T2 m2 = K::ld_nc2(Mq + 2 * C + c), m3 = K::ld_nc2(Mq + 3 * C + c);
