@@ -201,6 +201,47 @@ def run_peaks(args):
                       "derived_fp32_tflops_148sm_128lanes_1965mhz": FP32_PEAK_TFLOPS, "library": B.aera_version()}), flush=True)
 
 
+def run_sizes(args):
+    """--sizes: aera_unfold_batch at N = 1024 / 2048 / 4096 in both precisions (30-80 MHz table, fs = 200 MHz, ~1 GB of
+    seeded random traces per case, inputs and outputs >> L2), the dispatched kernel against the generic one: one JSON
+    line per (dtype, N). Not a BASELINE workload; it shows what a user at another trace length gets."""
+    import torch
+    import paper_1507_07733_b200.binding as B
+    torch.cuda.set_device(0)
+    hbm, src = load_peaks()
+    grid = ai.WORKLOADS[0].grid
+    fs = args.fs_mhz * 1e6 if args.fs_mhz > 0 else 200e6
+    for dtype, N in (("f32", 1024), ("f64", 1024), ("f32", 2048), ("f64", 2048), ("f32", 4096), ("f64", 4096)):
+        td = torch.float32 if dtype == "f32" else torch.float64
+        H = ai.pattern_table(grid, np.complex64 if dtype == "f32" else np.complex128)
+        pat = B.aera_pattern_upload(B.make_desc(grid, B.AERA_F32 if dtype == "f32" else B.AERA_F64), H)
+        S = 100
+        E = int(1.0e9 / (S * 2 * N * (4 if dtype == "f32" else 8)))
+        g = torch.Generator(device="cuda"); g.manual_seed(7733)
+        tr = torch.randn(E, S, 2, N, dtype=td, device="cuda", generator=g)
+        dirs = torch.rand(E, 2, dtype=torch.float64, device="cuda", generator=g) * torch.tensor([60.0, 360.0], device="cuda", dtype=torch.float64)
+        ef = torch.empty_like(tr); amp = torch.empty(E, S, dtype=td, device="cuda"); idx = torch.empty(E, S, dtype=torch.int32, device="cuda")
+        ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_UNFOLD, pat, B.AERA_F32 if dtype == "f32" else B.AERA_F64, E, S, N, fs))
+        rec = {"dtype": dtype, "n_samples": N, "fs_hz": fs, "units": E * S, "algorithmic_bytes_per_unit": 4 * N * tr.element_size() + tr.element_size() + 4}
+        for variant, key in ((0, "dispatched"), (1, "generic")):
+            B.aera_set_kernel_variant(variant)
+            for _ in range(max(args.warmup, 3)):
+                B.aera_unfold_batch(pat, tr, dirs, fs, efield=ef, peak_amp=amp, peak_idx=idx, workspace=ws)
+            torch.cuda.synchronize()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            n = max(args.steps // 2, 5); e0.record()
+            for _ in range(n):
+                B.aera_unfold_batch(pat, tr, dirs, fs, efield=ef, peak_amp=amp, peak_idx=idx, workspace=ws)
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / n
+            gbs = rec["units"] * rec["algorithmic_bytes_per_unit"] / (ms * 1e-3) / 1e9
+            rec[key] = {"kernel": B.aera_last_kernel(), "units_per_s": rec["units"] / (ms * 1e-3), "ms_per_step": ms, "GB_per_s": gbs, "frac_of_hbm_peak": gbs / hbm}
+        B.aera_set_kernel_variant(0)
+        rec["hbm_peak_gbs"] = hbm; rec["hbm_source"] = src
+        print(json.dumps(rec), flush=True)
+        pat.free(); del tr, ef, ws
+
+
 SCAN_FLOPS_PER_PAIR = 180000  # SURVEY 8(d-3): solve + two pruned inverse transforms + envelope per (direction, station)
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz (DESIGN.md 5.1)
 
@@ -450,6 +491,7 @@ def main():
     ap.add_argument("--loop", type=int, default=0, help="config 1 only: time the device-resident reconstruction loop with this many iterations")
     ap.add_argument("--fold", action="store_true", help="time the on-device forward model (aera_fold_batch) on the config's shapes")
     ap.add_argument("--peaks", action="store_true", help="measure and print the device's ALU issue peaks (packed fp32, fp32, fp64) and exit")
+    ap.add_argument("--sizes", action="store_true", help="throughput of the dispatched and the generic kernels at N = 1024 / 2048 / 4096, fp32 and fp64 (one JSON line each) and exit")
     ap.add_argument("--i16", action="store_true", help="int16 ADC-count input (aera_unfold_batch_i16): 24 584 algorithmic bytes per unit at configs[1]")
     ap.add_argument("--patterns", type=int, default=1, help="number of resident antenna-pattern tables, stations assigned round-robin (aera_unfold_batch_multi)")
     ap.add_argument("--fs-mhz", type=float, default=0.0, help="variant of the config at another sampling rate (another band-row geometry; not a BASELINE workload)")
@@ -471,6 +513,10 @@ def main():
     if args.peaks:
         if int(os.environ.get("RANK", "0")) == 0:
             run_peaks(args)
+        return
+    if args.sizes:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_sizes(args)
         return
 
     if args.config == 2:
