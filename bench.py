@@ -673,10 +673,23 @@ def main():
         if world > 1:
             t = torch.tensor([t_e2e], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); t_e2e = float(t.item())
         same = bool(torch.equal(out_idx, d_idx[:ne_h].cpu()))
+        # the floor of this leg: the same bytes copied in both directions at once (two streams, no kernel)
+        d_in = torch.empty(host_tr.shape, dtype=host_tr.dtype, device="cuda")
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize(); tc = time.perf_counter()
+        for _ in range(n_e2e):
+            with torch.cuda.stream(s_in):
+                d_in.copy_(host_tr, non_blocking=True)
+            with torch.cuda.stream(s_out):
+                out_ef.copy_(d_ef[:ne_h], non_blocking=True)
+        torch.cuda.synchronize()
+        t_copy = (time.perf_counter() - tc) / n_e2e
+        del d_in
         e2e = {"value": world * ne_h * wl.n_stations / t_e2e, "unit": UNIT, "n_events": int(ne_h), "h2d_bytes_per_step": int(host_tr.numel() * host_tr.element_size() + dirs_h.numel() * 8),
                "d2h_bytes_per_step": int(out_ef.numel() * out_ef.element_size() + out_amp.numel() * out_amp.element_size() + out_idx.numel() * 4),
                "ms_per_step": t_e2e * 1e3, "steps": n_e2e, "api": "aera_unfold_batch_host (pinned host buffers, 3-stream chunk pipeline)",
-               "matches_device_path": same}
+               "matches_device_path": same, "copy_only_ms": t_copy * 1e3, "frac_of_copy_only": t_copy / t_e2e,
+               "copy_only_note": "the step's H2D and D2H bytes copied concurrently on two streams with no kernel: the PCIe floor of this leg on this box"}
         del out_ef
 
     # ---- CPU oracle baseline on the box's host cores (rank 0, N=1 only), bounded sample
