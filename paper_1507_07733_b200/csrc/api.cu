@@ -507,7 +507,7 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     // up-sampling runs on the generic kernels (the specialised ones transform on the input grid only)
     const bool fast = kernel_variant() == 0 && ext.upsample == 1;
     const bool warp_path = fast && w32_supported(dtype, pl->dev);
-    const bool team_path = fast && !ext.input_i16 && t4k_supported(dtype, pl->dev);
+    const bool team_path = fast && t4k_supported(dtype, pl->dev);   // (int16 input: fp32 only, which aera_unfold_batch_i16 guarantees)
     const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
     const int team_warps = team_path ? t4k_team_warps(dtype, pl->dev) : 0;
     const int layout = warp_path ? MINV_PACKED_PAD

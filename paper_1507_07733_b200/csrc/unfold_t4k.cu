@@ -76,7 +76,7 @@ constexpr int kCtlF64 = 512;                          // TMEM base, per-team pea
 template <typename T>
 struct T4kParams {
     using T2 = typename T4k<T>::T2;
-    const T *traces;
+    const void *traces;   // T [n_units][2][N], or int16 ADC counts of the same shape (IN16; the counts-to-volts factors are in Minv)
     T *efield;
     T *amp;
     int32_t *idx;
@@ -177,7 +177,7 @@ __device__ __forceinline__ void fft1024_d(T (&P)[32], T (&Q)[32], T *X, const T2
     }
 }
 
-template <typename T, int TW, int RLO, int RHI, bool HAS_EF, int kTeams>
+template <typename T, int TW, int RLO, int RHI, bool HAS_EF, int kTeams, bool IN16>
 __global__ void __launch_bounds__(kTeams *TW * 32, 1)
 unfold_t4k_kernel(T4kParams<T> p)
 {
@@ -225,12 +225,20 @@ unfold_t4k_kernel(T4kParams<T> p)
 
 #pragma unroll 1
     for (long u = u0 + team; u < u1; u += kTeams) {
-        const T *v = p.traces + (size_t)u * 2 * N;
+        const T *v = static_cast<const T *>(p.traces) + (size_t)u * 2 * N;
+        const int16_t *v16 = static_cast<const int16_t *>(p.traces) + (size_t)u * 2 * N;
+        auto ldv = [&](int i) -> T {   // sample i of the station's [2][N] block
+            if constexpr (IN16) { short c; asm volatile("ld.global.nc.L1::no_allocate.s16 %0, [%1];" : "=h"(c) : "l"(v16 + i)); return (T)c; }
+            else return K::ld_stream(v + i);
+        };
         T *ef = HAS_EF ? p.efield + (size_t)u * 2 * N : nullptr;
         const long ev = u / p.n_stations;
         const T2 *M = p.minv + (size_t)ev * ((size_t)(4 * TW) * ((p.k_hi >> kLogTW) - (p.k_lo >> kLogTW) + 1)) +
                            (p.pattern_id ? (size_t)p.pattern_id[u - ev * p.n_stations] * p.minv_pattern_stride : 0);
-        if (w == 0 && lane == 0 && u + kTeams < u1) prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(T));
+        if (w == 0 && lane == 0 && u + kTeams < u1) {
+            if (IN16) prefetch_l2_bulk(v16 + (size_t)kTeams * 2 * N, 2 * N * sizeof(int16_t));
+            else prefetch_l2_bulk(v + (size_t)kTeams * 2 * N, 2 * N * sizeof(T));
+        }
 
         T P[32], Q[32];
         // ---- a1 + radix-TW step: thread holds y_q[m], q = 0..TW-1, m = lane + 32 (MPW w + jj), at [MPW q + jj]
@@ -238,10 +246,10 @@ unfold_t4k_kernel(T4kParams<T> p)
         static_for<0, 8>([&](auto jc) {
             constexpr int jj = decltype(jc)::value;
             const int m = lane + 32 * (8 * w + jj);
-            const T x0r = K::ld_stream(v + m), x1r = K::ld_stream(v + m + 1024);
-            const T x2r = K::ld_stream(v + m + 2048), x3r = K::ld_stream(v + m + 3072);
-            const T x0i = K::ld_stream(v + N + m), x1i = K::ld_stream(v + N + m + 1024);
-            const T x2i = K::ld_stream(v + N + m + 2048), x3i = K::ld_stream(v + N + m + 3072);
+            const T x0r = ldv(m), x1r = ldv(m + 1024);
+            const T x2r = ldv(m + 2048), x3r = ldv(m + 3072);
+            const T x0i = ldv(N + m), x1i = ldv(N + m + 1024);
+            const T x2i = ldv(N + m + 2048), x3i = ldv(N + m + 3072);
             const T ar = x0r + x2r, ai = x0i + x2i, br = x0r - x2r, bi = x0i - x2i;
             const T cr = x1r + x3r, ci = x1i + x3i, dr = x1r - x3r, di = x1i - x3i;
             P[jj] = ar + cr; Q[jj] = ai + ci;                    // y0
@@ -261,8 +269,8 @@ unfold_t4k_kernel(T4kParams<T> p)
         static_for<0, 16>([&](auto jc) {
             constexpr int jj = decltype(jc)::value;
             const int m = lane + 32 * (16 * w + jj);
-            const T x0r = K::ld_stream(v + m), x1r = K::ld_stream(v + m + 1024);
-            const T x0i = K::ld_stream(v + N + m), x1i = K::ld_stream(v + N + m + 1024);
+            const T x0r = ldv(m), x1r = ldv(m + 1024);
+            const T x0i = ldv(N + m), x1i = ldv(N + m + 1024);
             P[jj] = x0r + x1r; Q[jj] = x0i + x1i;               // y0
             const T y1r = x0r - x1r, y1i = x0i - x1i;
             const T2 w1 = TQ[m];                            // W_2048^m, m < 1024
@@ -272,8 +280,8 @@ unfold_t4k_kernel(T4kParams<T> p)
         } else {   // one warp holds the whole station: straight into FFT input order, no exchange
         static_for<0, 32>([&](auto jc) {
             constexpr int j = decltype(jc)::value;
-            P[brev5(j)] = K::ld_stream(v + lane + 32 * j);
-            Q[brev5(j)] = K::ld_stream(v + N + lane + 32 * j);
+            P[brev5(j)] = ldv(lane + 32 * j);
+            Q[brev5(j)] = ldv(N + lane + 32 * j);
         });
         }
 
@@ -509,12 +517,12 @@ unfold_t4k_kernel(T4kParams<T> p)
     if (warp == 0) tmem_free_all(*tmem_base);
 }
 
-template <typename T, int TW, int RLO, int RHI, bool HAS_EF>
+template <typename T, int TW, int RLO, int RHI, bool HAS_EF, bool IN16 = false>
 cudaError_t launch_t4k(const T4kParams<T> &q, cudaStream_t s)
 {
     constexpr int kTeams = kTeamsOf<T> * 4 / TW;       // the same warps per CTA for every team size
     const size_t smem = (size_t)kTabF64 + kCtlF64 + (size_t)kTeams * TW * kPlaneBytes;
-    auto kern = unfold_t4k_kernel<T, TW, RLO, RHI, HAS_EF, kTeams>;
+    auto kern = unfold_t4k_kernel<T, TW, RLO, RHI, HAS_EF, kTeams, IN16>;
     AERA_ENSURE_DYN_SMEM(kern, smem);
     long grid = (q.n_units + kTeams - 1) / kTeams;
     if (grid > sm_count()) grid = sm_count();
@@ -528,7 +536,7 @@ cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, con
 {
     using T2 = typename T4k<T>::T2;
     T4kParams<T> q;
-    q.traces = (const T *)traces; q.efield = (T *)efield; q.amp = (T *)amp; q.idx = idx;
+    q.traces = traces; q.efield = (T *)efield; q.amp = (T *)amp; q.idx = idx;
     q.minv = (const T2 *)minv; q.tw1024 = (const T2 *)p.tw1024; q.twN = (const T2 *)p.twN;
     q.n_units = n_units; q.n_stations = n_stations; q.k_lo = p.k_lo; q.k_hi = p.k_hi; q.K = p.K;
     q.pattern_id = x.pattern_id; q.minv_pattern_stride = x.minv_pattern_stride;
@@ -538,6 +546,12 @@ cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, con
     const bool r412 = (p.k_lo / (32 * tw)) == 4 && (p.k_hi / (32 * tw)) == 12;
     auto pick = [&](auto twc) -> cudaError_t {
         constexpr int TWc = decltype(twc)::value;
+        if constexpr (sizeof(T) == 4) {   // int16 ADC counts in, fp32 out (aera_unfold_batch_i16)
+            if (x.input_i16) {
+                if (r412) return efield ? launch_t4k<T, TWc, 4, 12, true, true>(q, s) : launch_t4k<T, TWc, 4, 12, false, true>(q, s);
+                return efield ? launch_t4k<T, TWc, 0, 15, true, true>(q, s) : launch_t4k<T, TWc, 0, 15, false, true>(q, s);
+            }
+        }
         if (r412) return efield ? launch_t4k<T, TWc, 4, 12, true>(q, s) : launch_t4k<T, TWc, 4, 12, false>(q, s);
         return efield ? launch_t4k<T, TWc, 0, 15, true>(q, s) : launch_t4k<T, TWc, 0, 15, false>(q, s);
     };

@@ -100,3 +100,25 @@ def test_upsampled_matches_oracle(B, cfg, events, n_st, u):
     E, S = tr.shape[:2]
     ref = ox.unfold_batch_upsampled(wl.grid, H, wl.fs_hz, tr.reshape(E * S, 2, -1), np.repeat(dirs, S, axis=0), u)
     _check(wl, compare(wl.dtype, ef.cpu().numpy().reshape(E * S, 2, -1), amp.cpu().numpy().ravel(), idx.cpu().numpy().ravel(), ref), f"upsampled x{u} cfg{cfg}")
+
+
+@pytest.mark.parametrize("N,fs,kernel", [(4096, 200e6, "unfold_t4k_f32"), (4096, 250e6, "unfold_t4k_f32"), (1024, 200e6, "unfold_t1k_f32")])
+def test_int16_input_on_the_team_kernels(B, N, fs, kernel):
+    """int16 ADC counts at the other register-resident trace lengths (fp32 out): the team kernel's templated load."""
+    from oracle import aera_ext as ox
+    base = ai.WORKLOADS[0]
+    wl = ai.Workload(96, "i16-team", 2, 9, N, fs, "f32", base.grid, 60.0, N // 4, 3 * N // 4, 5.0)
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    tr, dirs, _, _ = ai.make_batch(wl, range(2))
+    g = (0.0625, 0.05)
+    counts = np.stack([np.clip(np.round(tr[:, :, c] / g[c]), -32768, 32767) for c in (0, 1)], axis=2).astype(np.int16)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        ef, amp, idx = B.aera_unfold_batch_i16(pat, torch.from_numpy(counts).cuda(), g, torch.from_numpy(dirs).cuda(), fs)
+        torch.cuda.synchronize()
+        assert B.aera_last_kernel() == kernel and ef.dtype == torch.float32
+    finally:
+        pat.free()
+    E, S = counts.shape[:2]
+    ref = ox.unfold_batch_i16(wl.grid, H, fs, counts.reshape(E * S, 2, -1), g, np.repeat(dirs, S, axis=0), want_env2=True)
+    _check(wl, compare("f32", ef.cpu().numpy().reshape(E * S, 2, -1), amp.cpu().numpy().ravel(), idx.cpu().numpy().ravel(), ref), f"int16 N={N} {kernel}")
