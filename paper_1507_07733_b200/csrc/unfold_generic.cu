@@ -256,6 +256,7 @@ scan_inverse_generic_kernel(PlanDev p, int n_stations, long n_pairs, const cx<T>
 
 size_t elem_bytes(int dtype) { return dtype == AERA_F32 ? sizeof(cx<float>) : sizeof(cx<double>); }
 bool fits_smem(int dtype, int N, int U = 1) { return ((size_t)N + 2 * (size_t)N * U) * elem_bytes(dtype) <= kSmemBudget; }
+int generic_threads(int N) { const int t = N / 4; return t < 32 ? 32 : (t > kThreads ? kThreads : t); }
 long generic_grid(long n_units) { return n_units < (long)sm_count() * 4 ? n_units : (long)sm_count() * 4; }
 
 template <typename K>
@@ -269,12 +270,17 @@ cudaError_t launch_unfold_t(int dtype, const PlanDev &p, long n_units, int n_sta
                             void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s, const UnfoldExt &x)
 {
     ProfScope prof(KID_UNFOLD, s);
-    const long grid = generic_grid(n_units);
+    // short traces: fewer threads per CTA and more CTAs per SM (256 threads on 64 points leave three quarters of them
+    // idle at every barrier; measured fp32 N = 64 / 128 / 256 / 512: 182 / 307 / 498 / 502 -> 551 / 601 / 651 / 553 GB/s)
+    const int threads = generic_threads(p.N);
+    const long per_sm = 2048 / threads > 32 ? 32 : 2048 / threads;
+    const long small_grid = n_units < (long)sm_count() * per_sm ? n_units : (long)sm_count() * per_sm;
+    const long grid = threads < kThreads ? small_grid : generic_grid(n_units);   // (the workspace slices of the long sizes are per generic_grid CTA)
     if (fits_smem(dtype, p.N, p.U)) {
         size_t smem = ((size_t)p.N + 2 * (size_t)p.N * p.U) * sizeof(cx<T>);
         cudaError_t e = set_smem(unfold_generic_kernel<T, true, IN>, smem);
         if (e != cudaSuccess) return e;
-        unfold_generic_kernel<T, true, IN><<<(unsigned)grid, kThreads, smem, s>>>(
+        unfold_generic_kernel<T, true, IN><<<(unsigned)grid, threads, smem, s>>>(
             p, n_units, n_stations, (const IN *)traces, (T *)efield, (T *)amp, idx, (const cx<T> *)minv, nullptr,
             x.pattern_id, x.minv_pattern_stride);
     } else {
