@@ -202,7 +202,7 @@ def run_peaks(args):
 
 
 def run_sizes(args):
-    """--sizes: aera_unfold_batch at N = 1024 / 2048 / 4096 in both precisions (30-80 MHz table, fs = 200 MHz, ~1 GB of
+    """--sizes: aera_unfold_batch at N = 1024 ... 16384 in both precisions (30-80 MHz table, fs = 200 MHz, ~1 GB of
     seeded random traces per case, inputs and outputs >> L2), the dispatched kernel against the generic one: one JSON
     line per (dtype, N). Not a BASELINE workload; it shows what a user at another trace length gets."""
     import torch
@@ -211,7 +211,8 @@ def run_sizes(args):
     hbm, src = load_peaks()
     grid = ai.WORKLOADS[0].grid
     fs = args.fs_mhz * 1e6 if args.fs_mhz > 0 else 200e6
-    for dtype, N in (("f32", 1024), ("f64", 1024), ("f32", 2048), ("f64", 2048), ("f32", 4096), ("f64", 4096)):
+    for dtype, N in (("f32", 1024), ("f64", 1024), ("f32", 2048), ("f64", 2048), ("f32", 4096), ("f64", 4096),
+                     ("f32", 8192), ("f64", 8192), ("f32", 16384)):
         td = torch.float32 if dtype == "f32" else torch.float64
         H = ai.pattern_table(grid, np.complex64 if dtype == "f32" else np.complex128)
         pat = B.aera_pattern_upload(B.make_desc(grid, B.AERA_F32 if dtype == "f32" else B.AERA_F64), H)

@@ -82,13 +82,13 @@ cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_
 //   MINV_Q4     : per direction 16 planes [q = k & 3][entry 0..3 as in MINV_ROWS][C] complex, column
 //                 (k >> 2) - (k_lo >> 2), C = (k_hi >> 2) - (k_lo >> 2) + 1; slots of bins outside the
 //                 band are never written or used                                       (team kernel, teams of 4 warps)
-//   MINV_Q2, MINV_Q1 : the same with q = k & 1 (8 planes) / q = 0 (4 planes, C = K)    (teams of 2 warps / 1 warp)
+//   MINV_Q2, MINV_Q1, MINV_Q8, MINV_Q16 : the same with q = k mod 2 / 1 / 8 / 16 (4 tw planes)  (teams of 2 / 1 / 8 / 16 warps)
 //   MINV_Q32    : per direction 64 float4 planes [q = k & 31][A | B as in MINV_PACKED][C], column
 //                 (k >> 5) - (k_lo >> 5), C = (k_hi >> 5) - (k_lo >> 5) + 1              (long-trace kernel)
 //   MINV_PACKED_PAD : MINV_PACKED with 32 zero entries before and after each plane (planes of K + 64 entries, bin j at
 //                 index j + 32): a warp kernel whose edge rows reach up to 31 bins beyond the band multiplies by zero
 //                 there instead of clamping the index and selecting                       (batch warp kernel)
-enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3, MINV_PACKED_PAD = 4, MINV_Q2 = 5, MINV_Q1 = 6 };
+enum MinvLayout { MINV_ROWS = 0, MINV_PACKED = 1, MINV_Q4 = 2, MINV_Q32 = 3, MINV_PACKED_PAD = 4, MINV_Q2 = 5, MINV_Q1 = 6, MINV_Q8 = 7, MINV_Q16 = 8 };
 constexpr int kMinvPad = 32;
 // complex elements per direction in the MINV_Q4 / Q2 / Q1 layouts, tw = 4 / 2 / 1 (<= 4 K + 8 tw)
 __host__ __device__ inline size_t minv_qt_stride(int tw, int k_lo, int k_hi) { return (size_t)4 * tw * ((k_hi / tw) - (k_lo / tw) + 1); }

@@ -340,6 +340,8 @@ static const char *team_kernel_name(int dtype, int team_warps)
 {
     if (team_warps == 4) return dtype == AERA_F64 ? "unfold_t4k_f64" : "unfold_t4k_f32";
     if (team_warps == 2) return dtype == AERA_F64 ? "unfold_t2k_f64" : "unfold_t2k_f32";
+    if (team_warps == 8) return dtype == AERA_F64 ? "unfold_t8k_f64" : "unfold_t8k_f32";
+    if (team_warps == 16) return "unfold_t16k_f32";
     return dtype == AERA_F64 ? "unfold_t1k_f64" : "unfold_t1k_f32";
 }
 
@@ -511,7 +513,7 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
     const bool long_path = fast && !ext.input_i16 && long_f32_supported(dtype, pl->dev);
     const int team_warps = team_path ? t4k_team_warps(dtype, pl->dev) : 0;
     const int layout = warp_path ? MINV_PACKED_PAD
-                                 : (team_path ? (team_warps == 4 ? MINV_Q4 : (team_warps == 2 ? MINV_Q2 : MINV_Q1)) : (long_path ? MINV_Q32 : MINV_ROWS));
+                                 : (team_path ? (team_warps == 4 ? MINV_Q4 : (team_warps == 2 ? MINV_Q2 : (team_warps == 8 ? MINV_Q8 : (team_warps == 16 ? MINV_Q16 : MINV_Q1)))) : (long_path ? MINV_Q32 : MINV_ROWS));
     // complex elements of one event's matrices in this layout; the tables' slabs follow one another
     const size_t per_event = team_path ? minv_qt_stride(team_warps, pl->dev.k_lo, pl->dev.k_hi)
                              : (layout == MINV_Q32 ? (size_t)128 * ((pl->dev.k_hi >> 5) - (pl->dev.k_lo >> 5) + 1)

@@ -158,8 +158,8 @@ minv_kernel(const cx<T> *__restrict__ table, TableGeom g, const double *__restri
         }
         if (layout == MINV_ROWS) {
             o[0] = mt0; o[1] = mt1; o[2] = mp0; o[3] = mp1;
-        } else if (layout == MINV_Q4 || layout == MINV_Q2 || layout == MINV_Q1) {
-            const int tw = layout == MINV_Q4 ? 4 : (layout == MINV_Q2 ? 2 : 1);
+        } else if (layout == MINV_Q4 || layout == MINV_Q2 || layout == MINV_Q1 || layout == MINV_Q8 || layout == MINV_Q16) {
+            const int tw = layout == MINV_Q4 ? 4 : (layout == MINV_Q2 ? 2 : (layout == MINV_Q8 ? 8 : (layout == MINV_Q16 ? 16 : 1)));
             const int k = k_lo + j, C = ((k_lo + K - 1) / tw) - (k_lo / tw) + 1;
             cx<T> *q = minv + (size_t)d * 4 * tw * C + (size_t)(k % tw) * 4 * C + ((k / tw) - (k_lo / tw));
             q[0] = mt0; q[C] = mt1; q[2 * C] = mp0; q[3 * C] = mp1;

@@ -177,13 +177,39 @@ __device__ __forceinline__ void fft1024_d(T (&P)[32], T (&Q)[32], T *X, const T2
     }
 }
 
+// R-point forward DFT (R = 2^LOGR <= 32) of the values in (re[i], im[i]), input element j at position brev(j) over LOGR
+// bits, output in natural order: the first LOGR stages of fft32's butterfly network (same twiddle indices in units of
+// 2 pi / 32). Called with (im, re) it is the un-normalised inverse.
+template <class Ln, int LOGR, typename T>
+__device__ __forceinline__ void fft_pow2(T *re, T *im)
+{
+    static_for<0, LOGR>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        constexpr int half = 1 << s;
+        static_for<0, (1 << LOGR) / 2>([&](auto bc) {
+            constexpr int b = decltype(bc)::value;
+            constexpr int j = b & (half - 1);
+            constexpr int i0 = ((b - j) << 1) + j;
+            constexpr int i1 = i0 + half;
+            constexpr int idx = j * (16 >> s);
+            butterfly<Ln, idx>(re[i0], im[i0], re[i1], im[i1]);
+        });
+    });
+}
+__host__ __device__ constexpr int brev_n(int j, int bits)
+{
+    int r = 0;
+    for (int b = 0; b < bits; ++b) r |= ((j >> b) & 1) << (bits - 1 - b);
+    return r;
+}
+
 template <typename T, int TW, int RLO, int RHI, bool HAS_EF, int kTeams, bool IN16>
 __global__ void __launch_bounds__(kTeams *TW * 32, 1)
 unfold_t4k_kernel(T4kParams<T> p)
 {
     using T2 = typename T4k<T>::T2;
     using K = T4k<T>;
-    static_assert(TW == 1 || TW == 2 || TW == 4, "team of 1, 2 or 4 warps");
+    static_assert(TW == 1 || TW == 2 || TW == 4 || TW == 8 || TW == 16, "team of 1, 2, 4, 8 or 16 warps");
     static_assert(kTeams * TW <= 16 && (TW == 1 || kTeams <= 15), "tensor-memory column blocks / named barriers");
     constexpr int N = 1024 * TW;
     constexpr int MPW = 32 / TW;                    // values of m per thread in the radix-TW step
@@ -199,10 +225,10 @@ unfold_t4k_kernel(T4kParams<T> p)
     uint32_t *tmem_base = reinterpret_cast<uint32_t *>(smem + kTabF64);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
-    constexpr int kLogTW = TW == 4 ? 2 : (TW == 2 ? 1 : 0);
+    constexpr int kLogTW = TW == 16 ? 4 : (TW == 8 ? 3 : (TW == 4 ? 2 : (TW == 2 ? 1 : 0)));
     const int team = warp >> kLogTW, w = warp & (TW - 1);   // (shifts and masks: a signed division hides w's range from the compiler)
-    T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + (TW == 1 ? 0 : team) * 4;   // [team][4]
-    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + (TW == 1 ? 0 : kTeams) * 32) + team * 4;   // (unused when TW = 1)
+    T *peak_v = reinterpret_cast<T *>(smem + kTabF64 + 64) + (TW == 1 ? 0 : team) * (TW < 4 ? 4 : TW);   // [team][TW]
+    int *peak_i = reinterpret_cast<int *>(smem + kTabF64 + 64 + (TW == 1 ? 0 : (TW > 4 ? 4 : kTeams)) * 32) + (TW == 1 ? 0 : team) * (TW < 4 ? 4 : TW);   // (unused when TW = 1)
     unsigned char *tb = smem + kTabF64 + kCtlF64 + (size_t)team * kRegionX;
     T *RX = reinterpret_cast<T *>(tb);            // region X
     T *XW = RX + (size_t)w * (kPlaneBytes / 8);        // this warp's transpose plane
@@ -264,6 +290,30 @@ unfold_t4k_kernel(T4kParams<T> p)
             t = y1r * w1.x; P[8 + jj] = fma(y1i, -w1.y, t); t = y1r * w1.y; Q[8 + jj] = fma(y1i, w1.x, t);
             t = y2r * w2.x; P[16 + jj] = fma(y2i, -w2.y, t); t = y2r * w2.y; Q[16 + jj] = fma(y2i, w2.x, t);
             t = y3r * w3.x; P[24 + jj] = fma(y3i, -w3.y, t); t = y3r * w3.y; Q[24 + jj] = fma(y3i, w3.x, t);
+        });
+        } else if constexpr (TW >= 8) {   // radix-TW step as a small register FFT over j'; W_N^{q m} by powers of W_N^m
+        static_for<0, MPW>([&](auto jc) {
+            constexpr int jj = decltype(jc)::value;
+            const int m = lane + 32 * (MPW * w + jj);
+            T xr[TW], xi[TW];
+            static_for<0, TW>([&](auto tc) {
+                constexpr int j = decltype(tc)::value;
+                xr[brev_n(j, kLogTW)] = ldv(m + 1024 * j);
+                xi[brev_n(j, kLogTW)] = ldv(N + m + 1024 * j);
+            });
+            fft_pow2<typename K::Lane, kLogTW>(xr, xi);
+            const T2 w1 = TQ[m];                            // W_N^m, m < 1024
+            T2 wq = w1;
+            P[jj] = xr[0]; Q[jj] = xi[0];
+            static_for<1, TW>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                T t = xr[q] * wq.x; P[MPW * q + jj] = fma(xi[q], -wq.y, t);
+                t = xr[q] * wq.y; Q[MPW * q + jj] = fma(xi[q], wq.x, t);
+                if constexpr (q + 1 < TW) {
+                    const T nr = fma(wq.x, w1.x, -(wq.y * w1.y)), ni = fma(wq.x, w1.y, wq.y * w1.x);
+                    wq.x = nr; wq.y = ni;
+                }
+            });
         });
         } else if constexpr (TW == 2) {
         static_for<0, 16>([&](auto jc) {
@@ -393,8 +443,13 @@ unfold_t4k_kernel(T4kParams<T> p)
             fft1024_d(Q, P, XW, TW_, lane);                        // inverse: roles swapped; u_q[m = lane + 32 b] in (P[b], Q[b])
             if (w != 0) {
                 // u_q[m] conj(W_4096^{q m}), m = lane + 32 b: two interleaved recurrences over b (ratio W^{64 q})
-                const T2 r2 = w4096<TW>(TQ, 64 * w);
-                const T2 c0 = w4096<TW>(TQ, (w * lane) & (N - 1)), c1 = w4096<TW>(TQ, (w * (lane + 32)) & (N - 1));
+                T2 r2, c0, c1;
+                if constexpr (TW >= 8) {   // three values per transform: straight from the plan's full table W_N^t
+                    r2 = p.twN[(64 * w) & (N - 1)]; c0 = p.twN[(w * lane) & (N - 1)]; c1 = p.twN[(w * (lane + 32)) & (N - 1)];
+                } else {
+                    r2 = w4096<TW>(TQ, 64 * w);
+                    c0 = w4096<TW>(TQ, (w * lane) & (N - 1)); c1 = w4096<TW>(TQ, (w * (lane + 32)) & (N - 1));
+                }
                 T er = c0.x, ei = c0.y, orr = c1.x, oi = c1.y;
                 static_for<0, 32>([&](auto bc) {
                     constexpr int b = decltype(bc)::value;
@@ -441,6 +496,21 @@ unfold_t4k_kernel(T4kParams<T> p)
                     const T ar = P[jj], ai = Q[jj];
                     P[jj] = ar + P[16 + jj]; Q[jj] = ai + Q[16 + jj];
                     P[16 + jj] = ar - P[16 + jj]; Q[16 + jj] = ai - Q[16 + jj];
+                });
+            }
+            if constexpr (TW >= 8) {
+                static_for<0, MPW>([&](auto jc) {
+                    constexpr int jj = decltype(jc)::value;
+                    T xr[TW], xi[TW];
+                    static_for<0, TW>([&](auto qc) {
+                        constexpr int q = decltype(qc)::value;
+                        xr[brev_n(q, kLogTW)] = P[MPW * q + jj]; xi[brev_n(q, kLogTW)] = Q[MPW * q + jj];
+                    });
+                    fft_pow2<typename K::Lane, kLogTW>(xi, xr);          // inverse: roles swapped
+                    static_for<0, TW>([&](auto sc2) {
+                        constexpr int sidx = decltype(sc2)::value;
+                        P[MPW * sidx + jj] = xr[sidx]; Q[MPW * sidx + jj] = xi[sidx];
+                    });
                 });
             }
             if constexpr (TW == 4)
@@ -556,6 +626,10 @@ cudaError_t launch_t4k_typed(const PlanDev &p, long n_units, int n_stations, con
         return efield ? launch_t4k<T, TWc, 0, 15, true>(q, s) : launch_t4k<T, TWc, 0, 15, false>(q, s);
     };
     if (tw == 1) return pick(IC<1>{});
+    if (tw == 8) return pick(IC<8>{});
+    if constexpr (sizeof(T) == 4) {     // (sixteen fp64 warps of 250 registers do not fit an SM)
+        if (tw == 16) return pick(IC<16>{});
+    }
     if constexpr (sizeof(T) == 8) {     // (fp32 N = 2048 is the warp kernel's)
         if (tw == 2) return pick(IC<2>{});
     }
@@ -570,6 +644,8 @@ int t4k_team_warps(int dtype, const PlanDev &p)
     if (p.N == 4096 && (dtype == AERA_F64 || dtype == AERA_F32)) return 4;
     if (p.N == 2048 && dtype == AERA_F64) return 2;
     if (p.N == 1024 && (dtype == AERA_F64 || dtype == AERA_F32)) return 1;
+    if (p.N == 8192 && (dtype == AERA_F64 || dtype == AERA_F32)) return 8;
+    if (p.N == 16384 && dtype == AERA_F32) return 16;
     return 0;
 }
 bool t4k_supported(int dtype, const PlanDev &p) { return t4k_team_warps(dtype, p) != 0; }

@@ -23,7 +23,10 @@ def B():
                                                ("f32", 1024, 200e6, "unfold_t1k_f32"), ("f32", 1024, 180e6, "unfold_t1k_f32"),
                                                ("f64", 2048, 200e6, "unfold_t2k_f64"), ("f64", 2048, 250e6, "unfold_t2k_f64"),
                                                ("f64", 1024, 200e6, "unfold_t1k_f64"), ("f64", 1024, 180e6, "unfold_t1k_f64"),
-                                               ("f32", 512, 200e6, "generic"), ("f64", 8192, 200e6, "generic")])
+                                               ("f32", 8192, 200e6, "unfold_t8k_f32"), ("f32", 8192, 250e6, "unfold_t8k_f32"),
+                                               ("f64", 8192, 200e6, "unfold_t8k_f64"), ("f64", 8192, 180e6, "unfold_t8k_f64"),
+                                               ("f32", 16384, 200e6, "unfold_t16k_f32"), ("f32", 16384, 180e6, "unfold_t16k_f32"),
+                                               ("f32", 512, 200e6, "generic"), ("f64", 16384, 200e6, "generic")])
 def test_batch_other_bands(B, dtype, N, fs, kernel):
     import oracle
     base = ai.WORKLOADS[0]
@@ -111,7 +114,8 @@ def test_spectrum_reuse_on_another_band_is_bit_identical(B):
         pat.free()
 
 
-@pytest.mark.parametrize("dtype,N,kernel", [("f64", 1024, "unfold_t1k_f64"), ("f64", 2048, "unfold_t2k_f64"), ("f32", 1024, "unfold_t1k_f32")])
+@pytest.mark.parametrize("dtype,N,kernel", [("f64", 1024, "unfold_t1k_f64"), ("f64", 2048, "unfold_t2k_f64"), ("f32", 1024, "unfold_t1k_f32"),
+                                            ("f32", 8192, "unfold_t8k_f32"), ("f64", 8192, "unfold_t8k_f64"), ("f32", 16384, "unfold_t16k_f32")])
 def test_team_sizes_fold_inplace_peaks_only_and_tables(B, dtype, N, kernel):
     """Teams of one and two warps (N = 1024 / 2048) through every entry point that shares the team kernel: the forward
     model against the oracle's fold, E-field written over the traces, peaks only, and two identical tables reproducing

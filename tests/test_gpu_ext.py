@@ -102,7 +102,7 @@ def test_upsampled_matches_oracle(B, cfg, events, n_st, u):
     _check(wl, compare(wl.dtype, ef.cpu().numpy().reshape(E * S, 2, -1), amp.cpu().numpy().ravel(), idx.cpu().numpy().ravel(), ref), f"upsampled x{u} cfg{cfg}")
 
 
-@pytest.mark.parametrize("N,fs,kernel", [(4096, 200e6, "unfold_t4k_f32"), (4096, 250e6, "unfold_t4k_f32"), (1024, 200e6, "unfold_t1k_f32")])
+@pytest.mark.parametrize("N,fs,kernel", [(4096, 200e6, "unfold_t4k_f32"), (4096, 250e6, "unfold_t4k_f32"), (1024, 200e6, "unfold_t1k_f32"), (8192, 200e6, "unfold_t8k_f32")])
 def test_int16_input_on_the_team_kernels(B, N, fs, kernel):
     """int16 ADC counts at the other register-resident trace lengths (fp32 out): the team kernel's templated load."""
     from oracle import aera_ext as ox

@@ -35,7 +35,8 @@ CASES = [  # dtype, N, fs, events, stations, expected kernel
     ("f32", 2048, 180e6, 3, 37, "unfold_w32"), ("f32", 2048, 200e6, 2, 13, "unfold_w32"), ("f32", 2048, 500e6, 2, 5, "unfold_w32"),
     ("f64", 4096, 200e6, 2, 7, "unfold_t4k_f64"), ("f32", 4096, 250e6, 2, 9, "unfold_t4k_f32"),
     ("f64", 2048, 200e6, 3, 5, "unfold_t2k_f64"), ("f64", 1024, 250e6, 3, 11, "unfold_t1k_f64"), ("f32", 1024, 200e6, 1, 19, "unfold_t1k_f32"),
-    ("f32", 65536, 1e9, 1, 3, "unfold_long_f32"), ("f32", 256, 200e6, 2, 7, "generic"), ("f64", 8192, 200e6, 1, 2, "generic"),
+    ("f32", 65536, 1e9, 1, 3, "unfold_long_f32"), ("f32", 256, 200e6, 2, 7, "generic"), ("f64", 16384, 200e6, 1, 2, "generic"),
+    ("f32", 8192, 200e6, 2, 5, "unfold_t8k_f32"), ("f64", 8192, 250e6, 1, 3, "unfold_t8k_f64"), ("f32", 16384, 180e6, 1, 3, "unfold_t16k_f32"),
 ]
 
 
