@@ -119,7 +119,12 @@ cudaError_t launch_unfold_w32(const PlanDev &p, long n_events, int n_stations, c
 
 // ---- unfold_t4k.cu: team-per-station kernel, N = 1024 x (warps of a team): 4096 fp64 (configs[3]) / fp32, 2048 fp64, 1024 fp64 / fp32
 bool t4k_supported(int dtype, const PlanDev &p);
-int t4k_team_warps(int dtype, const PlanDev &p);   // 4, 2, 1, or 0 when the kernel does not cover (dtype, N, band)
+int t4k_team_warps(int dtype, const PlanDev &p);
+// (the fp32 and the int16-input instantiations live in their own translation units, unfold_t4k_f32.cu / unfold_t4k_i16.cu)
+cudaError_t launch_unfold_t4k_i16(const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield, void *amp,
+                                  int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x);
+cudaError_t launch_unfold_t4k_f32(const PlanDev &p, long n_units, int n_stations, const void *traces, void *efield, void *amp,
+                                  int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x);   // 4, 2, 1, or 0 when the kernel does not cover (dtype, N, band)
 cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                   void *amp, int32_t *idx, const void *minv, cudaStream_t s, const UnfoldExt &x = UnfoldExt());
 
