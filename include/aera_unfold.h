@@ -306,9 +306,11 @@ aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches)
 aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count, int *sm_clock_khz);
 
 /* Which kernel family the most recent aera_unfold_batch / aera_fold_batch / aera_scan_directions /
- * aera_reconstruct_batch call of this thread dispatched to: a static string such as "unfold_w32<10,28>",
- * "unfold_t4k_f64", "unfold_long_f32", "scan_w32", "generic" ("" before the first call). Lets a caller see that a
- * size or band fell to the slower generic radix-2 kernels. */
+ * aera_reconstruct_batch call of this thread dispatched to: a static string, one of "unfold_w32" (fp32 N = 2048),
+ * "unfold_t1k_f32|f64" (N = 1024), "unfold_t2k_f64" (N = 2048), "unfold_t4k_f32|f64" (N = 4096), "unfold_t8k_f32|f64"
+ * (N = 8192), "unfold_t16k_f32" (N = 16384), "unfold_long_f32" (fp32 N = 65536, band below N/4), "scan_w32" (fp32
+ * N = 2048 scan), "generic" (every other size, and up-sampling); "" before the first call. Lets a caller see that a
+ * size fell to the slower generic radix-8 kernels. */
 const char *aera_last_kernel(void);
 
 /* Message for the most recent non-OK status on this thread ("" if none). Static storage. */

@@ -1,8 +1,10 @@
 // Team-per-station fused unfolding kernel for N = 4096, fp64 (BASELINE configs[3]) and fp32 (the same code on plain
 // float lanes: a user with 4096-sample fp32 traces gets a register-resident path instead of the generic radix-8 one).
 // The team size TW is a template parameter: N = 1024 TW, TW = 4 (described below), 2 (N = 2048: a radix-2 step across
-// two warps) or 1 (N = 1024: one warp per station, no team exchange), so fp64 traces of 1024 / 2048 samples and fp32
-// traces of 1024 samples stay register-resident too (fp32 N = 2048 is unfold_w32.cu's).
+// two warps), 1 (N = 1024: one warp per station, no team exchange), 8 and 16 (N = 8192 / 16384: the radix-TW step across
+// the team is a small register FFT, fft_pow2), so fp64 traces of 1024 / 2048 / 8192 samples and fp32 traces of
+// 1024 / 8192 / 16384 samples stay register-resident too (fp32 N = 2048 is unfold_w32.cu's). IN16 reads int16 ADC counts.
+// Instantiated in unfold_t4k.cu (fp64 + dispatch), unfold_t4k_f32.cu and unfold_t4k_i16.cu.
 //
 // A "team" of 4 warps (128 threads x 32 complex doubles = 128 registers each) holds one station
 // entirely in registers; a CTA runs 2 teams (8 warps, one CTA per SM, persistent). Every long
