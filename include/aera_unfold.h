@@ -114,6 +114,9 @@ size_t aera_workspace_bytes(aera_op_t op, const aera_pattern_t *pattern, int dty
  * All buffers are caller-owned. n_samples: power of two in [64, 65536]. The result is linear in
  * the traces; units are the caller's (configs: microvolt in, microvolt/metre out).
  * NaN/Inf in the data are not checked (they propagate). n_events == 0 is a no-op.
+ * Side effect on the device: the first call with n_samples = 65536 (fp32) raises cudaLimitPersistingL2CacheSize to the
+ * device maximum for the rest of the process (the long-trace kernel's scratch must stay in the L2; environment variable
+ * AERA_LONG_PERSIST_MB=0 leaves the limit alone, =<n> sets n MB). Nothing else changes device-wide state.
  * Errors: INVALID_ARG, UNSUPPORTED_N, DTYPE_MISMATCH, WORKSPACE, BAND, ALLOC (first-use plan), CUDA. */
 aera_status_t aera_unfold_batch(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
                                 int n_samples, double fs_hz, const void *traces, const double *dirs,
