@@ -282,6 +282,54 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
                                      const double *dirs_host, void *efield_host, void *peak_amp_host,
                                      int32_t *peak_idx_host);
 
+/*
+ * Batch unfolding without a workspace and without any allocation (the operation of aera_unfold_batch; PAPER.md
+ * section 2, L29 steps 3 + 4; section 5: keep the data on the device and the copies out of the loop).
+ *
+ * For whom: code that is handed its input and output buffers and nothing else. Two cases in practice. (1) A
+ * reconstruction module loaded into a host application that owns the device-memory pool: the module may not call
+ * cudaMalloc, and often could not if it tried because the pool has taken the whole card. (2) A trigger or
+ * monitoring loop with a latency budget: cudaMalloc / cudaFree serialise on a driver lock and synchronise the
+ * device, so one allocation anywhere in the loop stalls every stream of the process.
+ *
+ * The scratch that aera_unfold_batch takes as `workspace` is here an array of AERA_STATIC_SCRATCH_BYTES (32 MiB)
+ * built into the library. Every GPU on which the library's code is loaded holds those 32 MiB until the process
+ * exits, whether this call is used or not. A batch whose aera_workspace_bytes(AERA_OP_UNFOLD, ...) exceeds the
+ * array is refused with AERA_ERR_WORKSPACE (the message gives both numbers); nothing is allocated instead. At
+ * BASELINE configs[1] (n_samples = 2048 fp32, fs = 180 MHz) one event needs 20 256 bytes, so up to 1 656 events
+ * fit in a call; cut larger batches into several calls.
+ *
+ * Arguments are those of aera_unfold_batch without workspace / workspace_bytes; results are the same bit for bit
+ * (the same kernels run). The call itself makes no cudaMalloc, cudaFree or other allocating call, on the host or
+ * on the device. Two things therefore belong to set-up:
+ *   - aera_pattern_prepare(pattern, n_samples, fs_hz, stream) once per (pattern, n_samples, fs_hz): it builds the
+ *     small plan (twiddle and bin tables) that the other entry points build on first use, which is a cudaMalloc and
+ *     a synchronising upload. Without it this call returns AERA_ERR_INVALID_ARG and says so.
+ *   - the FIRST call of this entry point on each device looks up the device address of the built-in array (and the
+ *     CUDA runtime loads the kernels' code on first launch). Make that first call with that device current, during
+ *     set-up, and before any stream capture is begun; later calls on that device do a table look-up only.
+ *     Leave aera_profile_enable off (it creates events).
+ * All calls on one device share the one array, and it keeps whatever the previous call wrote. Nothing in it needs
+ * to start at zero (each call writes every entry it later reads), so consecutive calls on ONE stream are safe as
+ * they are. Two calls that can overlap on the GPU -- different streams, or different host threads without ordering
+ * between their streams -- race on the array and produce garbage: order them (one stream, or events), or give the
+ * second one a workspace of its own through aera_unfold_batch.
+ * Errors: as aera_unfold_batch, plus the two above.
+ */
+#define AERA_STATIC_SCRATCH_BYTES (32u << 20)
+aera_status_t aera_unfold_batch_static(const aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                       int n_samples, double fs_hz, const void *traces, const double *dirs,
+                                       void *efield, void *peak_amp, int32_t *peak_idx, void *cuda_stream);
+
+/* Set-up for aera_unfold_batch_static (useful before any entry point when the first hot call must not allocate or
+ * synchronise): builds and caches the plan of (n_samples, fs_hz) in the pattern handle. Allocates device memory and
+ * synchronises the stream once; a second call for the same pair is a no-op. Errors: INVALID_ARG, UNSUPPORTED_N, BAND,
+ * ALLOC, CUDA. */
+aera_status_t aera_pattern_prepare(aera_pattern_t *pattern, int n_samples, double fs_hz, void *cuda_stream);
+
+/* AERA_STATIC_SCRATCH_BYTES as the loaded library was built (for bindings that cannot read the macro). */
+size_t aera_static_scratch_bytes(void);
+
 /* Kernel selection, for tests and tuning. 0 = automatic (specialised kernels where available),
  * 1 = always the generic radix-2 kernel. Process-wide. Returns the previous value. */
 int aera_set_kernel_variant(int variant);

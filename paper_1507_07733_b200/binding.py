@@ -22,7 +22,8 @@ STATUS = {0: "AERA_OK", 1: "AERA_ERR_INVALID_ARG", 2: "AERA_ERR_UNSUPPORTED_N", 
 EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_workspace_bytes", "aera_unfold_batch",
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel", "aera_unfold_batch_multi", "aera_unfold_batch_i16",
-           "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex", "aera_reconstruct_convergence")
+           "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex", "aera_reconstruct_convergence",
+           "aera_unfold_batch_static", "aera_pattern_prepare", "aera_static_scratch_bytes")
 
 
 class AeraError(RuntimeError):
@@ -94,6 +95,11 @@ def _load():
     lib.aera_reconstruct_convergence.argtypes = [dp, C.c_int, C.c_int, C.c_double, vp, vp]
     lib.aera_reconstruct_convergence.restype = C.c_int
     lib.aera_last_kernel.restype = C.c_char_p
+    lib.aera_unfold_batch_static.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp, vp]
+    lib.aera_unfold_batch_static.restype = C.c_int
+    lib.aera_pattern_prepare.argtypes = [vp, C.c_int, C.c_double, vp]
+    lib.aera_pattern_prepare.restype = C.c_int
+    lib.aera_static_scratch_bytes.restype = C.c_size_t
     lib.aera_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), ip, ip]
     lib.aera_measure_alu_peak.restype = C.c_int
     lib.aera_version.restype = C.c_char_p
@@ -258,6 +264,32 @@ def aera_unfold_batch(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_h
         workspace = alloc_workspace(aera_workspace_bytes(AERA_OP_UNFOLD, p, dt, E, S, N, fs_hz) if E > 0 else 256, traces.device)
     _check(_lib.aera_unfold_batch(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp),
                                   _ptr(peak_idx), _ptr(workspace), workspace.numel(), _stream_ptr(stream)))
+    return efield, peak_amp, peak_idx
+
+
+def aera_static_scratch_bytes() -> int:
+    """Size of the scratch array built into the library (the limit of aera_unfold_batch_static)."""
+    return int(_lib.aera_static_scratch_bytes())
+
+
+def aera_pattern_prepare(p: Pattern, n_samples: int, fs_hz: float, stream=None):
+    """Set-up: build the plan of (n_samples, fs_hz) now (allocates, synchronises) so that later calls do not."""
+    _check(_lib.aera_pattern_prepare(p.handle, int(n_samples), float(fs_hz), _stream_ptr(stream)))
+
+
+def aera_unfold_batch_static(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor, fs_hz: float, efield, peak_amp, peak_idx, stream=None):
+    """aera_unfold_batch on the library's built-in scratch array, for callers that may not allocate device memory:
+    no workspace argument, and EVERY output is the caller's (efield may be None for peaks only) -- this wrapper
+    allocates nothing either. Needs aera_pattern_prepare(p, N, fs_hz) beforehand; batches whose scratch exceeds
+    aera_static_scratch_bytes() raise AeraError (AERA_ERR_WORKSPACE). Calls that overlap on the GPU race on the array."""
+    E, S, two, N = traces.shape
+    assert two == 2 and traces.is_cuda and traces.is_contiguous()
+    assert dirs.is_cuda and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    assert peak_amp is not None and peak_idx is not None and tuple(peak_amp.shape) == (E, S) and tuple(peak_idx.shape) == (E, S)
+    assert peak_amp.dtype == traces.dtype and peak_idx.dtype == torch.int32 and peak_amp.is_contiguous() and peak_idx.is_contiguous()
+    assert efield is None or (efield.shape == traces.shape and efield.dtype == traces.dtype and efield.is_contiguous())
+    _check(_lib.aera_unfold_batch_static(p.handle, _dtype_code(traces.dtype), E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield),
+                                         _ptr(peak_amp), _ptr(peak_idx), _stream_ptr(stream)))
     return efield, peak_amp, peak_idx
 
 

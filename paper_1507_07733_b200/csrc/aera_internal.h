@@ -73,6 +73,12 @@ int sm_count();
 // records the kernel family a call dispatched to (aera_last_kernel)
 void note_kernel(const char *name);
 
+// ---- api.cu hooks of unfold_static.cu (aera_unfold_batch_static)
+// sets the thread's aera_last_error() message and returns st
+aera_status_t report_error(aera_status_t st, const char *msg);
+// whether the plan of (n_samples, fs_hz), up-sampling 1, is already built: a look-up, never a build
+bool plan_is_cached(const aera_pattern_t *pattern, int n_samples, double fs_hz);
+
 // ---- pattern.cu
 cudaError_t launch_repack(int dtype, const void *src, void *dst, int n_z, int n_a, int n_f, cudaStream_t s);
 // Minv[d][j][4] = scale * H(theta_d, phi_d, f_{k_lo+j})^-1.

@@ -816,3 +816,23 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
 }
 
 } // extern "C"
+
+// ---- set-up call and hooks of aera_unfold_batch_static (unfold_static.cu)
+namespace aera {
+aera_status_t report_error(aera_status_t st, const char *msg) { return fail(st, "%s", msg); }
+bool plan_is_cached(const aera_pattern_t *pattern, int n_samples, double fs_hz)
+{
+    aera_pattern *pat = const_cast<aera_pattern *>(pattern);
+    std::lock_guard<std::mutex> lk(pat->mu);
+    return pat->plans.find(std::make_pair((long long)n_samples | (1LL << 32), fs_hz)) != pat->plans.end();
+}
+} // namespace aera
+
+extern "C" aera_status_t aera_pattern_prepare(aera_pattern_t *pattern, int n_samples, double fs_hz, void *cuda_stream)
+{
+    if (!pattern) return fail(AERA_ERR_INVALID_ARG, "pattern is NULL");
+    aera_status_t st = check_n(n_samples);
+    if (st != AERA_OK) return st;
+    Plan *pl = nullptr;
+    return get_plan(pattern, n_samples, fs_hz, static_cast<cudaStream_t>(cuda_stream), &pl);
+}
