@@ -195,7 +195,16 @@ def run_peaks(args):
     torch.cuda.set_device(0)
     sampler = ClockSampler(0); sampler.start()
     pk = measure_alu_peaks(B)
+    t_end = time.time() + 1.0                               # keep the SMs busy long enough for nvidia-smi to see the clock under load
+    while time.time() < t_end:
+        B.aera_measure_alu_peak(B.ALU_KINDS["f32x2"], 16)
     clocks = sampler.stop()
+    # sm_clock_mhz above is the device's MAXIMUM SM clock (cudaDevAttrClockRate): the per-clock figures derived from it
+    # understate the pipe under throttling; these use the clock nvidia-smi observed during the measurement
+    if clocks.get("sm_mhz"):
+        for v in pk.values():
+            v["sm_clock_mhz_observed"] = clocks["sm_mhz"]
+            v["lane_fma_per_observed_clk_per_sm"] = v["lane_fma_per_s"] / v["sm_count"] / (clocks["sm_mhz"] * 1e6)
     hbm, src = load_peaks()
     print(json.dumps({"alu_peaks": pk, "hbm_gbs": hbm, "hbm_source": src, "clocks": clocks,
                       "derived_fp32_tflops_148sm_128lanes_1965mhz": FP32_PEAK_TFLOPS, "library": B.aera_version()}), flush=True)

@@ -144,8 +144,11 @@ aera_status_t aera_scan_directions(const aera_pattern_t *pattern, int dtype, int
  * k_hi - k_lo + 1): E[k] = weights[k - k_lo] * H[k]^-1 V[k], e.g. a band-pass taper or notches at narrow-band
  * transmitters. The weights are folded into the per-direction matrices, so the filter costs nothing per
  * station. It applies to aera_unfold_batch, aera_scan_directions and aera_reconstruct_batch of this pattern
- * for that (n_samples, fs_hz) until replaced; weights == NULL removes it. aera_fold_batch ignores it.
- * weights is a HOST pointer; the call synchronises the stream (it is a configuration call, not a hot one).
+ * for that (n_samples, fs_hz) until replaced; weights == NULL removes it. The multi-table, int16 and up-sampled
+ * variants apply it too (up-sampling does not change the band: z[upsample * n] stays sample n of the filtered
+ * aera_unfold_batch). aera_fold_batch ignores it.
+ * weights is a HOST pointer. A configuration call, not a hot one: it synchronises the whole DEVICE (no kernel of an
+ * earlier call on any stream may still be reading the old weights) and then the stream for the upload.
  */
 aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_samples, double fs_hz, const double *weights,
                                            int n_weights, void *cuda_stream);
@@ -175,7 +178,9 @@ aera_status_t aera_fold_batch(const aera_pattern_t *pattern, int dtype, int n_ev
  * patterns[pattern_id[s]]; the per-direction matrices are then built once per (event, table).
  *   patterns    HOST array of n_patterns handles (1..64), all of the call's dtype and with the same frequency axis
  *               (n_freq, freq0_hz, dfreq_hz: the in-band bins must agree); zenith / azimuth grids may differ
- *   pattern_id  DEVICE [n_stations] int32, values in 0 .. n_patterns-1 (not checked on the device)
+ *   pattern_id  DEVICE [n_stations] int32, values in 0 .. n_patterns-1. The call is asynchronous and the array is on the
+ *               device, so a value outside that range cannot be reported: it is clamped to the nearest valid table
+ *               (a negative id uses table 0, a too large one the last table) and never indexes outside the workspace
  *   workspace   >= aera_workspace_bytes_ex(AERA_OP_UNFOLD, patterns[0], dtype, n_events, n_stations, n_samples, fs_hz,
  *               n_patterns, 1)
  * A band filter set on patterns[0] applies to all tables. Errors as aera_unfold_batch.
@@ -352,7 +357,10 @@ aera_status_t aera_profile_read(int kernel_id, double *total_ms, long *launches)
  * on every SM (warps_per_sm warps each, 1..32) is timed with CUDA events (best of 3).
  *   kind 0: packed fp32 (fma.rn.f32x2, the warp kernels' instruction), 1: scalar fp32, 2: fp64
  *   lane_fma_per_s  out: fused multiply-adds per second over the whole device (x 2 = FLOP/s)
- *   sm_count, sm_clock_khz  out: cudaDevAttrMultiProcessorCount, cudaDevAttrClockRate (may be NULL)
+ *   sm_count, sm_clock_khz  out: cudaDevAttrMultiProcessorCount, cudaDevAttrClockRate (may be NULL). The latter is the
+ *                           device's MAXIMUM SM clock, not the clock during the measurement: a per-clock figure derived
+ *                           from it understates the pipe when the device throttles (bench.py --peaks also reports one on
+ *                           the clock nvidia-smi observed)
  * SYNCHRONOUS (default stream); allocates and frees a small device buffer. Errors: INVALID_ARG, ALLOC/CUDA. */
 aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count, int *sm_clock_khz);
 

@@ -51,11 +51,17 @@ def unfold_batch_i16(grid, H, fs_hz: float, counts, counts_to_volts, dirs, want_
     return _o.unfold_batch(grid, H, fs_hz, v, dirs, want_env2=want_env2)
 
 
-def unfold_station_upsampled(grid, H, fs_hz: float, v, theta_deg: float, phi_deg: float, upsample: int):
-    """One station, analytic signal on a grid `upsample` times finer. -> dict(efield [2][uN], env2 [uN], amp, idx)."""
+def unfold_station_upsampled(grid, H, fs_hz: float, v, theta_deg: float, phi_deg: float, upsample: int, weights=None):
+    """One station, analytic signal on a grid `upsample` times finer. -> dict(efield [2][uN], env2 [uN], amp, idx).
+    weights (optional, [K] real): the pre-filter of oracle/aera_filter.py, E'[k] = w[k - k_lo] E[k], applied to the band
+    spectra before the fine-grid transform (the band, hence the weights, do not depend on the up-sampling factor)."""
     u = int(upsample)
     assert u >= 1
     r = _o.unfold_station_spectra(grid, H, fs_hz, v, theta_deg, phi_deg)       # O1-O4: the band spectra E_theta, E_phi
+    if weights is not None:
+        w = np.asarray(weights, dtype=np.float64)
+        assert w.shape == r["Et"].shape
+        r = dict(r, Et=r["Et"] * w, Ep=r["Ep"] * w)
     N = np.asarray(v).shape[-1]
     M = u * N
     # O5 on the fine grid: oracle.analytic_from_band(E, M, ...) = (2/M) sum_k E[k] exp(+2 pi i n k / M); times u gives 2/N
@@ -65,8 +71,8 @@ def unfold_station_upsampled(grid, H, fs_hz: float, v, theta_deg: float, phi_deg
     return dict(efield=np.stack([zt.real, zp.real]), env2=env2, amp=amp, idx=idx)
 
 
-def unfold_batch_upsampled(grid, H, fs_hz: float, traces, dirs, upsample: int):
+def unfold_batch_upsampled(grid, H, fs_hz: float, traces, dirs, upsample: int, weights=None):
     """traces [U][2][N], dirs [U][2] -> dict(efield [U][2][uN], env2 [U][uN], amp [U], idx [U])."""
-    rs = [unfold_station_upsampled(grid, H, fs_hz, traces[i], dirs[i][0], dirs[i][1], upsample) for i in range(len(traces))]
+    rs = [unfold_station_upsampled(grid, H, fs_hz, traces[i], dirs[i][0], dirs[i][1], upsample, weights) for i in range(len(traces))]
     return dict(efield=np.stack([r["efield"] for r in rs]), env2=np.stack([r["env2"] for r in rs]),
                 amp=np.array([r["amp"] for r in rs]), idx=np.array([r["idx"] for r in rs], dtype=np.int32))

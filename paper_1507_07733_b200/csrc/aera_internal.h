@@ -54,21 +54,34 @@ struct ProfScope {
     ~ProfScope() { prof_end(kid, s); }
 };
 
-// cudaFuncAttributeMaxDynamicSharedMemorySize raised once per kernel (and again only if a call needs more), not
-// on every launch: `cur` is a static of the call site, one per kernel instantiation.
+// Function attributes, device limits and device properties belong to ONE device: what the library remembers about them
+// is kept per device ordinal, so a process may use the library on several GPUs (one after the other or from several
+// threads, each with its own current device).
+constexpr int kMaxDevices = 64;
+// slot of the current device in such a table, or -1 (unknown / beyond the table: nothing is remembered for it)
+inline int device_slot()
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return -1; }
+    return (dev >= 0 && dev < kMaxDevices) ? dev : -1;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize raised once per kernel and device (and again only if a call needs more),
+// not on every launch: the table is a static of the call site, one per kernel instantiation.
 #define AERA_ENSURE_DYN_SMEM(kern, bytes)                                                                   \
     do {                                                                                                    \
-        static std::atomic<size_t> aera_cur_smem{0};                                                        \
-        if ((size_t)(bytes) > aera_cur_smem.load(std::memory_order_acquire)) {                              \
+        static std::atomic<size_t> aera_cur_smem[::aera::kMaxDevices];                                      \
+        const int aera_slot = ::aera::device_slot();                                                        \
+        if (aera_slot < 0 || (size_t)(bytes) > aera_cur_smem[aera_slot].load(std::memory_order_acquire)) {  \
             cudaError_t aera_e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes)); \
             if (aera_e != cudaSuccess) return aera_e;                                                       \
-            aera_cur_smem.store((size_t)(bytes), std::memory_order_release);                                \
+            if (aera_slot >= 0) aera_cur_smem[aera_slot].store((size_t)(bytes), std::memory_order_release); \
         }                                                                                                   \
     } while (0)
 
 // ---- peaks.cu: measured ALU issue peaks (aera_measure_alu_peak)
 cudaError_t measure_alu_peak(int kind, int warps_per_sm, double *lane_fma_per_s, int *sm_count, int *sm_clock_khz);
-// number of SMs of the current device (cached; api.cu)
+// number of SMs of the current device (cached per device; api.cu)
 int sm_count();
 // records the kernel family a call dispatched to (aera_last_kernel)
 void note_kernel(const char *name);
@@ -103,6 +116,8 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
                         int forward = 0 /* 1: scale * H (forward model) instead of scale * H^-1 */,
                         double chan_scale0 = 1.0, double chan_scale1 = 1.0 /* per-channel input scale folded into the columns */);
 size_t minv_smem_bytes(int dtype, int n_f);
+// out[i] = pattern_id[i] clamped to 0 .. n_patterns-1 (device to device; aera_unfold_batch_multi)
+cudaError_t launch_clamp_pattern_id(const int32_t *pattern_id, int32_t *out, int n_stations, int n_patterns, cudaStream_t s);
 
 // ---- unfold_generic.cu
 size_t generic_scratch_bytes(int dtype, int N, long n_units, int upsample = 1);   // per-call global transform buffers (0 if smem-resident)

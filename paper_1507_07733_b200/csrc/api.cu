@@ -27,15 +27,16 @@ void note_kernel(const char *name) { g_last_kernel = name; }
 
 int sm_count()
 {
-    static std::atomic<int> cached{0};
-    int n = cached.load(std::memory_order_relaxed);
+    static std::atomic<int> cached[kMaxDevices];           // per device ordinal (zero = not asked yet)
+    const int slot = device_slot();
+    int n = slot >= 0 ? cached[slot].load(std::memory_order_relaxed) : 0;
     if (n > 0) return n;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
         (void)cudaGetLastError();
         n = 148; // B200
     }
-    cached.store(n, std::memory_order_relaxed);
+    if (slot >= 0) cached[slot].store(n, std::memory_order_relaxed);
     return n;
 }
 
@@ -88,7 +89,6 @@ struct Plan {
     PlanDev dev{};
     double fs = 0;
     void *blob = nullptr; // one device allocation holding every table of the plan
-    double *d_filter = nullptr; // optional per-bin pre-filter weights (aera_pattern_set_band_filter)
 };
 
 struct HostPipe { // staging for aera_unfold_batch_host
@@ -113,6 +113,9 @@ struct aera_pattern {
     std::mutex mu;        // plans and filter weights
     std::mutex pipe_mu;   // the host pipeline's staging buffers and streams: one aera_unfold_batch_host at a time per handle
     std::map<std::pair<long long, double>, Plan *> plans;   // key: (n_samples | up-sampling factor << 32, fs)
+    // optional per-bin pre-filter weights (aera_pattern_set_band_filter), device [K]; key: (n_samples, fs). The band does
+    // not depend on the up-sampling factor, so every plan of (n_samples, fs) points its dev.bin_w at the same weights
+    std::map<std::pair<long long, double>, double *> filters;
     HostPipe pipe;
 };
 
@@ -240,6 +243,8 @@ aera_status_t get_plan(aera_pattern *pat, int N, double fs, cudaStream_t s, Plan
     pl->dev.twN = b + off_twN;
     pl->dev.U = U; pl->dev.logM = ilog2(N * U);
     pl->dev.twU = U > 1 ? b + off_twU : b + off_tw;
+    auto flt = pat->filters.find(std::make_pair((long long)N, fs));
+    pl->dev.bin_w = flt != pat->filters.end() ? flt->second : nullptr;
     pat->plans[key] = pl;
     *out = pl;
     return AERA_OK;
@@ -254,7 +259,7 @@ TableGeom geom_of(const aera_pattern_desc_t &d)
 }
 
 struct WsLayout {
-    size_t off_minv, off_scratch, off_spectra, off_loop_spectra, off_peaks, total;
+    size_t off_minv, off_scratch, off_spectra, off_loop_spectra, off_peaks, off_pid, total;
 };
 
 // Workspace: [Minv: n_dirs*K*4 complex] [generic transform buffers] [scan: spectra S*2*K complex]
@@ -283,6 +288,8 @@ WsLayout ws_layout(aera_op_t op, int dtype, int N, int k_lo, int K, long n_dirs,
         o = align_up(o + w32_spectra_bytes(band, n_dirs * (long)n_stations));
     w.off_peaks = o;                                                      // fold: the by-product peaks of the shared kernels
     if (op == AERA_OP_FOLD) o = align_up(o + (size_t)n_dirs * n_stations * 12);
+    w.off_pid = o;                                                        // several tables: the range-checked copy of pattern_id
+    if (n_patterns > 1) o = align_up(o + (size_t)n_stations * sizeof(int32_t));
     w.total = o > 0 ? o : kAlign;
     return w;
 }
@@ -400,7 +407,8 @@ aera_status_t aera_pattern_upload(const aera_pattern_desc_t *desc, const void *H
 aera_status_t aera_pattern_free(aera_pattern_t *p)
 {
     if (!p) return AERA_OK;
-    for (auto &kv : p->plans) { cudaFree(kv.second->blob); cudaFree(kv.second->d_filter); delete kv.second; }
+    for (auto &kv : p->plans) { cudaFree(kv.second->blob); delete kv.second; }
+    for (auto &kv : p->filters) cudaFree(kv.second);
     HostPipe &hp = p->pipe;
     for (int i = 0; i < 2; ++i) {
         cudaFree(hp.d_in[i]); cudaFree(hp.d_out[i]); cudaFree(hp.d_amp[i]); cudaFree(hp.d_idx[i]);
@@ -438,19 +446,32 @@ aera_status_t aera_pattern_set_band_filter(aera_pattern_t *pattern, int n_sample
     std::lock_guard<std::mutex> lk(pattern->mu);
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return cuda_fail(e, "device synchronise");
-    if (!weights) { cudaFree(pl->d_filter); pl->d_filter = nullptr; pl->dev.bin_w = nullptr; return AERA_OK; }
+    const auto fkey = std::make_pair((long long)n_samples, fs_hz);
+    // every plan of this (n_samples, fs_hz), whatever its up-sampling factor, uses the same weights
+    auto point_plans_at = [&](const double *w) {
+        for (auto &kv : pattern->plans)
+            if ((kv.first.first & 0xffffffffLL) == (long long)n_samples && kv.first.second == fs_hz) kv.second->dev.bin_w = w;
+    };
+    auto cur = pattern->filters.find(fkey);
+    if (!weights) {
+        point_plans_at(nullptr);
+        if (cur != pattern->filters.end()) { cudaFree(cur->second); pattern->filters.erase(cur); }
+        return AERA_OK;
+    }
     if (n_weights != pl->dev.K)
         return fail(AERA_ERR_INVALID_ARG, "n_weights=%d but the band of (n_samples=%d, fs=%g) has %d bins (aera_band)", n_weights, n_samples, fs_hz, pl->dev.K);
     for (int j = 0; j < n_weights; ++j)
         if (!std::isfinite(weights[j])) return fail(AERA_ERR_INVALID_ARG, "weights[%d] is not finite", j);
-    if (!pl->d_filter) {
-        e = cudaMalloc((void **)&pl->d_filter, sizeof(double) * pl->dev.K);
-        if (e != cudaSuccess) { (void)cudaGetLastError(); pl->d_filter = nullptr; return fail(AERA_ERR_ALLOC, "cudaMalloc of the filter weights: %s", cudaGetErrorString(e)); }
+    double *d_w = cur != pattern->filters.end() ? cur->second : nullptr;
+    if (!d_w) {
+        e = cudaMalloc((void **)&d_w, sizeof(double) * pl->dev.K);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(AERA_ERR_ALLOC, "cudaMalloc of the filter weights: %s", cudaGetErrorString(e)); }
+        pattern->filters[fkey] = d_w;
     }
-    e = cudaMemcpyAsync(pl->d_filter, weights, sizeof(double) * pl->dev.K, cudaMemcpyHostToDevice, s);
+    e = cudaMemcpyAsync(d_w, weights, sizeof(double) * pl->dev.K, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "filter upload");
-    pl->dev.bin_w = pl->d_filter;
+    point_plans_at(d_w);
     return AERA_OK;
 }
 
@@ -520,6 +541,14 @@ static aera_status_t unfold_impl(const aera_pattern_t *pattern, int dtype, int n
                                                    : (layout == MINV_PACKED_PAD ? (size_t)(pl->dev.K + 2 * kMinvPad) * 4 : (size_t)pl->dev.K * 4));
     UnfoldExt x;
     x.pattern_id = ext.pattern_id;
+    if (ext.pattern_id && ext.n_patterns > 1) {   // the kernels index the matrix slabs with it: hand them a copy forced into range
+        int32_t *pid = reinterpret_cast<int32_t *>(ws + w.off_pid);
+        cudaError_t ce = launch_clamp_pattern_id(ext.pattern_id, pid, n_stations, ext.n_patterns, s);
+        if (ce != cudaSuccess) return cuda_fail(ce, "pattern_id range check launch");
+        x.pattern_id = pid;
+    } else if (ext.n_patterns == 1) {
+        x.pattern_id = nullptr;                    // one table: whatever the ids say, every station uses it
+    }
     x.minv_pattern_stride = (size_t)n_events * per_event;
     x.input_i16 = ext.input_i16;
     // the warp, team and long kernels form 2 V_c, so their matrix carries 1/N instead of 2/N

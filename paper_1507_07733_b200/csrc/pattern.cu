@@ -219,4 +219,21 @@ cudaError_t launch_minv(int dtype, const void *table, const TableGeom &g, const 
     return cudaGetLastError();
 }
 
+// aera_unfold_batch_multi: the antenna type of every station, forced into 0 .. n_patterns-1. The unfold kernels index the
+// per-table matrix slabs with these values; the caller's array lives on the device and the call is asynchronous, so a bad
+// value cannot be reported -- it is made harmless instead (clamped), and the kernels read this copy in the workspace.
+__global__ void clamp_pattern_id_kernel(const int32_t *__restrict__ in, int32_t *__restrict__ out, int n, int n_patterns)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = min(max(in[i], 0), n_patterns - 1);
+}
+
+cudaError_t launch_clamp_pattern_id(const int32_t *pattern_id, int32_t *out, int n_stations, int n_patterns, cudaStream_t s)
+{
+    if (n_stations <= 0) return cudaSuccess;
+    clamp_pattern_id_kernel<<<(unsigned)((n_stations + 255) / 256), 256, 0, s>>>(pattern_id, out, n_stations, n_patterns);
+    count_launches(1);
+    return cudaGetLastError();
+}
+
 } // namespace aera

@@ -275,8 +275,12 @@ cudaError_t launch_unfold_t(int dtype, const PlanDev &p, long n_units, int n_sta
     const int threads = generic_threads(p.N);
     const long per_sm = 2048 / threads > 32 ? 32 : 2048 / threads;
     const long small_grid = n_units < (long)sm_count() * per_sm ? n_units : (long)sm_count() * per_sm;
-    const long grid = threads < kThreads ? small_grid : generic_grid(n_units);   // (the workspace slices of the long sizes are per generic_grid CTA)
-    if (fits_smem(dtype, p.N, p.U)) {
+    // the global-scratch path has one slice per CTA of generic_grid (generic_scratch_bytes sizes it so): it must never
+    // run on the larger small_grid, which a short trace with a large up-sampling factor (N + 2 N U beyond shared
+    // memory, e.g. fp32 N = 512, U = 32) would otherwise select
+    const bool smem_path = fits_smem(dtype, p.N, p.U);
+    const long grid = (smem_path && threads < kThreads) ? small_grid : generic_grid(n_units);
+    if (smem_path) {
         size_t smem = ((size_t)p.N + 2 * (size_t)p.N * p.U) * sizeof(cx<T>);
         cudaError_t e = set_smem(unfold_generic_kernel<T, true, IN>, smem);
         if (e != cudaSuccess) return e;

@@ -488,7 +488,9 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
     auto launch = [&](auto kern) -> cudaError_t {
         AERA_ENSURE_DYN_SMEM(kern, smem);
         // persistent clusters: as many as can be co-resident (a cluster of 8 must fit one GPC), at most one per station
-        static int max_clusters = 0;                       // same for both instantiations to within rounding; cached
+        static std::atomic<int> max_clusters_of[kMaxDevices];   // cached per device (same for both instantiations to within rounding)
+        const int slot = device_slot();
+        int max_clusters = slot >= 0 ? max_clusters_of[slot].load(std::memory_order_relaxed) : 0;
         if (max_clusters == 0) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3(kLCluster * long_max_clusters()); cfg.blockDim = dim3(kLWarps * 32); cfg.dynamicSmemBytes = smem;
@@ -498,16 +500,16 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
             int n = 0;
             if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) { (void)cudaGetLastError(); n = long_max_clusters(); }
             max_clusters = n < long_max_clusters() ? n : long_max_clusters();
-            if (getenv("AERA_DEBUG")) fprintf(stderr, "[aera] long-trace kernel: %d co-resident clusters of %d CTAs (occupancy query %d)\n", max_clusters, kLCluster, n);
+            if (slot >= 0) max_clusters_of[slot].store(max_clusters, std::memory_order_relaxed);
         }
         const long clusters = n_units < max_clusters ? n_units : max_clusters;
         // The scratch lines carry an evict_last policy, which holds only inside the persisting carve-out of the L2: without
         // it a fifth of the scratch writes were evicted to DRAM before being overwritten (measured 1.83 MB of DRAM traffic
         // per station against 1.05 MB algorithmic, 1.146 M stations/s; with a 79 MB carve-out 1.11 MB, 1.116 M stations/s;
-        // with 70 MB = the scratch size 1.23 MB, 1.135 M stations/s). Set once per process to the device maximum (79 MB
+        // with 70 MB = the scratch size 1.23 MB, 1.135 M stations/s). Set once per process and device to the device maximum (79 MB
         // on the B200); AERA_LONG_PERSIST_MB=<n> overrides, 0 leaves the limit alone.
-        static std::atomic<int> persist_done{0};
-        if (!persist_done.exchange(1)) {
+        static std::atomic<int> persist_done[kMaxDevices];      // the limit is a property of the device: once per device
+        if (slot < 0 || !persist_done[slot].exchange(1)) {
             const char *ev = getenv("AERA_LONG_PERSIST_MB");
             int mx = 0, dev = 0;
             (void)cudaGetDevice(&dev);

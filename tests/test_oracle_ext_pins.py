@@ -85,6 +85,28 @@ def test_upsampled_grid_contains_the_original_samples_and_matches_scipy_resample
         assert np.all(up["amp"] >= base["amp"] * (1 - 1e-12))                                     # the fine grid can only find a higher peak
 
 
+def test_filtered_upsampled_contains_the_filtered_samples_and_matches_scipy_resample():
+    """The optional pre-filter weights of the up-sampling oracle: the fine grid through the filtered coarse samples
+    (oracle/aera_filter.py, pinned on its own), scipy's FFT resampling of them, and weights of one = no weights."""
+    from oracle import aera_filter as of
+    wl, H, tr, dirs = _setup(1)
+    dd = np.tile(dirs[0], (2, 1))
+    k_lo, k_hi = oracle.band(wl.n_samples, wl.fs_hz, wl.grid.n_freq, wl.grid.freq0_hz, wl.grid.dfreq_hz)
+    rng = np.random.default_rng(11)
+    w = 0.2 + 0.8 * rng.uniform(size=k_hi - k_lo + 1); w[[3, len(w) // 3, len(w) - 5]] = 0.0
+    base = of.unfold_batch_filtered(wl.grid, H, wl.fs_hz, tr[0, :2], dd, w)
+    plain = ox.unfold_batch_upsampled(wl.grid, H, wl.fs_hz, tr[0, :2], dd, 4)
+    ones = ox.unfold_batch_upsampled(wl.grid, H, wl.fs_hz, tr[0, :2], dd, 4, np.ones_like(w))
+    assert np.array_equal(plain["efield"], ones["efield"]) and np.array_equal(plain["idx"], ones["idx"])
+    up = ox.unfold_batch_upsampled(wl.grid, H, wl.fs_hz, tr[0, :2], dd, 4, w)
+    scale = np.abs(base["efield"]).max()
+    assert np.max(np.abs(up["efield"] - plain["efield"])) > 1e-3 * scale                         # the weights do something
+    assert np.max(np.abs(up["efield"][:, :, ::4] - base["efield"])) <= 1e-12 * scale
+    assert np.max(np.abs(up["env2"][:, ::4] - base["env2"])) <= 1e-12 * base["env2"].max()
+    ref = scipy.signal.resample(base["efield"], 4 * wl.n_samples, axis=-1)
+    assert np.max(np.abs(up["efield"] - ref)) <= 1e-11 * scale
+
+
 def test_upsampled_cosine_has_constant_envelope_and_half_sample_pulse_is_found():
     wl = ai.WORKLOADS[0]
     Hid = np.zeros(wl.grid.shape, dtype=np.complex128); Hid[0, 0] = 1.0; Hid[1, 1] = 1.0
