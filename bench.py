@@ -256,9 +256,10 @@ SCAN_FLOPS_PER_PAIR = 180000  # solve + two pruned inverse transf
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # 74.4: 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz
 
 
-def run_scan(args, wl):
+def run_scan(args, wl, emit=True):
     """--config 2: direction-hypothesis scan (one event, 124 stations, 41 x 180 directions). Unit = one
-    (direction, station) pair; FP32-pipe bound (no trace output), so the roofline block is "alu"."""
+    (direction, station) pair; FP32-pipe bound (no trace output), so the roofline block is "alu".
+    emit=False: return the JSON record instead of printing it (the default run's "also" array)."""
     import torch
     import torch.distributed as dist
     import paper_1507_07733_b200.binding as B
@@ -327,6 +328,17 @@ def run_scan(args, wl):
         out_a.copy_(amp, non_blocking=True); out_i.copy_(idx, non_blocking=True)
         torch.cuda.synchronize()
     t_e2e = (time.perf_counter() - t0) / n_e2e
+    # the oracle's scan on the host cores, bounded sample: the first 48 directions of this rank's list, every station
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        n_d = min(48, D)
+        t0 = time.perf_counter()
+        o_amp, o_idx = oracle.scan(wl.grid, H, wl.fs_hz, ev.traces, dirs_h[:n_d].numpy())
+        dt_o = time.perf_counter() - t0
+        cpu = {"value": n_d * S / dt_o, "unit": "pairs/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"first {n_d} directions x {S} stations of the timed scan ({n_d * S} pairs, {dt_o:.1f} s wall)",
+               "peak_idx_agreement_with_gpu": float(np.mean(o_idx == idx[:n_d].cpu().numpy()))}
     line = {
         "metric": "(direction, station) pairs scanned/sec (configs[2] scan mode; 2ch x 2048 fp32 per station)", "value": value_all,
         "unit": "pairs/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_all, "higher_is_better": True,
@@ -341,17 +353,83 @@ def run_scan(args, wl):
                      "algorithmic_flops_per_pair": SCAN_FLOPS_PER_PAIR,
                      "peak_source": f"measured in this run: aera_measure_alu_peak(fma.rn.f32x2) = {alu['lane_fma_per_clk_per_sm']:.1f} lane-FMA/clk/SM x {alu['sm_count']} SMs x {alu['sm_clock_mhz']:.0f} MHz x 2",
                      "derived_peak_tflops": FP32_PEAK_TFLOPS},
-        "cpu_baseline": None,
+        "cpu_baseline": cpu,
         "e2e": {"value": pairs / t_e2e, "unit": "pairs/s", "h2d_bytes_per_step": int(tr_h.numel() * 4 + dirs_h.numel() * 8),
                 "d2h_bytes_per_step": int(pairs * 8), "ms_per_step": t_e2e * 1e3, "steps": n_e2e},
         "gpu_launches": int(launches), "clocks": clocks, "outputs_sane": bool(np.isfinite(a).all()), "library": B.aera_version(),
     }
-    if rank == 0:
+    if rank == 0 and emit:
         print(json.dumps(line), flush=True)
     pat.free()
     if world > 1:
         dist.destroy_process_group()
+    return line
 
+
+def also_batch(B, cfg, steps, warmup, gpu_index=0):
+    """One compact device-resident record of a batch-unfold config at its BASELINE size (configs[3], configs[4]) for the
+    default run's "also" array: the same timing rules as the headline (warm-up, CUDA events on the launching stream
+    around `steps` steps, kernel time by events inside the library, clocks sampled during the timed region, inputs and
+    outputs far larger than the L2). The batch is a canonical block of seeded events tiled on the device."""
+    import torch
+    wl = ai.WORKLOADS[cfg]
+    dt_code = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt_code), H)
+    t0 = time.time()
+    n_events = wl.n_events
+    host_tr, d_tr, host_dirs, amp_inj, arr_inj = build_inputs_device(wl, n_events, 0, n_canon={3: 100, 4: 8}.get(cfg, 100))
+    d_dirs = host_dirs.cuda()
+    d_ef = torch.empty_like(d_tr)
+    d_amp = torch.empty((n_events, wl.n_stations), dtype=d_tr.dtype, device="cuda")
+    d_idx = torch.empty((n_events, wl.n_stations), dtype=torch.int32, device="cuda")
+    ws = B.alloc_workspace(B.aera_workspace_bytes(B.AERA_OP_UNFOLD, pat, dt_code, n_events, wl.n_stations, wl.n_samples, wl.fs_hz))
+    torch.cuda.synchronize()
+    setup_s = time.time() - t0
+    stream = torch.cuda.current_stream()
+    n_units = n_events * wl.n_stations
+
+    def step():
+        B.aera_unfold_batch(pat, d_tr, d_dirs, wl.fs_hz, efield=d_ef, peak_amp=d_amp, peak_idx=d_idx, workspace=ws, stream=stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(gpu_index); sampler.start()
+    B.aera_profile_enable(True)
+    l0 = B.aera_launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / steps
+    launches = B.aera_launch_count() - l0
+    B.aera_profile_enable(False)
+    k_ms, k_n = B.aera_profile_read(B.KERNEL_IDS["unfold"])
+    clocks = sampler.stop()
+    amp_h = d_amp.cpu().numpy(); idx_h = d_idx.cpu().numpy()
+    strong = amp_inj > 300.0
+    ok_idx = float(np.mean(np.abs(idx_h[strong] - arr_inj[strong]) <= 3))
+    peak, peak_src = load_peaks()
+    bytes_unit = algorithmic_bytes_per_unit(wl)
+    k_avg = k_ms / max(k_n, 1)
+    ach = n_units * bytes_unit / (k_avg * 1e-3) / 1e9
+    rec = {"metric": "station-traces unfolded/sec", "value": n_units / (ms_step * 1e-3), "unit": UNIT, "ms_per_step": ms_step, "steps": steps, "warmup": warmup,
+           "dtype": wl.dtype,
+           "config": {"workload": f"BASELINE configs[{wl.config}] {wl.name}: {n_events} events x {wl.n_stations} stations x 2 ch x {wl.n_samples} {wl.dtype}",
+                      "l2_policy": f"inputs+outputs {2 * d_tr.numel() * d_tr.element_size() / 1e9:.1f} GB per step >> 126 MB L2 (no flush needed)",
+                      "kernel": B.aera_last_kernel()},
+           "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "kernel_ms": k_avg,
+                        "kernel_share_of_step": k_avg / ms_step, "algorithmic_bytes_per_unit": bytes_unit, "peak_source": peak_src},
+           "gpu_launches": int(launches), "clocks": clocks,
+           "outputs_sane": bool(np.isfinite(amp_h).all() and ok_idx > (0.98 if wl.config != 4 else 0.6)), "strong_pulse_idx_within_3": ok_idx,
+           "setup_s": round(setup_s, 1)}
+    pat.free()
+    del d_tr, d_ef, d_amp, d_idx, ws
+    torch.cuda.empty_cache()
+    return rec
 
 
 def run_loop(args, wl):
@@ -508,6 +586,7 @@ def main():
     ap.add_argument("--samples", type=int, default=0, help="variant of the config at another trace length (not a BASELINE workload)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="default run only: skip the compact records of configs 2, 3 and 4 (the \"also\" array)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     wl = ai.WORKLOADS[args.config]
@@ -718,10 +797,9 @@ def main():
         cpu = {"value": U / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {n_ev_s} events x {n_st_s} stations of the timed batch ({U} units, {dt:.1f} s wall), OpenMP over units",
                "peak_idx_agreement_with_gpu": agree}
-        # the fairer O(N log N) CPU figure: the harness-side numpy float64 pipeline of tests/fastref.py
+        # the fairer O(N log N) CPU figure: the harness-side numpy float64 pipeline of fastref.py
         # (numpy.fft; pinned to the oracle in tests/test_fastref_vs_oracle.py), the closest analogue of the paper's
         # FFTW baseline; one event per task on a thread pool
-        sys.path.insert(0, os.path.join(ROOT, "tests"))
         import fastref
         n_thr = min(32, os.cpu_count() or 1)
         n_ev_f = min(host_tr.shape[0], {1: 1000, 3: 1000, 4: 16}[wl.config])
@@ -730,7 +808,7 @@ def main():
         rf = fastref.check_all_units(wl.grid, H, wl.fs_hz, tr_f, host_dirs[:n_ev_f].numpy(), None, amp_h[:n_ev_f], idx_h[:n_ev_f],
                                      {"tie": 1e-5 if wl.dtype == "f32" else 1e-10}, threads=n_thr)
         dtf = time.perf_counter() - t0
-        cpu["fft_numpy"] = {"value": n_ev_f * wl.n_stations / dtf, "unit": UNIT, "threads": n_thr, "kind": "numpy float64 rfft pipeline (tests/fastref.py), O(N log N)",
+        cpu["fft_numpy"] = {"value": n_ev_f * wl.n_stations / dtf, "unit": UNIT, "threads": n_thr, "kind": "numpy float64 rfft pipeline (fastref.py), O(N log N)",
                             "sample": f"first {n_ev_f} events of the timed batch ({n_ev_f * wl.n_stations} units, {dtf:.1f} s wall)",
                             "gpu_peak_idx": {"exact": rf["exact"], "tie_pm1": rf["tie_pm1"], "ambiguous": rf["ambiguous"], "miss": rf["miss"]},
                             "gpu_amp_max_rel_err": rf["max_amp"]}
@@ -748,6 +826,29 @@ def main():
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "outputs_sane": sane, "strong_pulse_idx_within_3": ok_idx, "setup_s": round(t_setup, 1), "library": B.aera_version(),
         }
+        # the other BASELINE configs at their stated sizes, a few timed steps each (north_star's target is stated on
+        # configs 1, 3 AND 4; the scan is config 2): only in the plain default run on one GPU
+        plain = (world == 1 and args.config == 1 and variant_note is None and args.variant == 0 and not args.events
+                 and not args.fs_mhz and not args.samples and not args.no_also)
+        if plain:
+            del d_tr, d_ef
+            torch.cuda.empty_cache()
+            also = []
+            k = max(3, min(args.steps, 10))
+            for cfg in (3, 4):
+                try:
+                    also.append(also_batch(B, cfg, k, 3, local_rank))
+                except Exception as e:   # a record that could not be measured says so; the headline stands
+                    also.append({"config": {"workload": f"BASELINE configs[{cfg}]"}, "error": repr(e)})
+            try:
+                import copy
+                a2 = copy.copy(args); a2.steps = k; a2.warmup = 3; a2.no_cpu_baseline = True
+                r = run_scan(a2, ai.WORKLOADS[2], emit=False)
+                also.append({key: r[key] for key in ("metric", "value", "unit", "ms_per_step", "steps", "warmup", "dtype", "config", "roofline",
+                                                      "gpu_launches", "clocks", "outputs_sane")})
+            except Exception as e:
+                also.append({"config": {"workload": "BASELINE configs[2]"}, "error": repr(e)})
+            line["also"] = also
         print(json.dumps(line), flush=True)
     pat.free()
     if world > 1:

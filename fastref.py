@@ -2,7 +2,8 @@
 SURVEY.md 8(c)-B, and the "fairer" CPU figure of 8(d-4) (the closest analogue of the paper's FFTW baseline,
 PAPER.md L31, L59).
 
-It is NOT the oracle and NOT the product: it lives in tests/, imports neither oracle/ nor the CUDA package, and
+It is NOT the oracle and NOT the product: harness code beside aera_inputs.py (used by tests/ and by bench.py's
+cpu_baseline leg), it imports neither oracle/ nor the CUDA package, and
 is trusted only because tests/test_fastref_vs_oracle.py pins it to the naive-DFT oracle (<= 1e-12 relative) on
 a subsample. Its job is coverage: the oracle costs O(N K) per unit and can only sample the big batches; this
 pipeline (numpy.fft in float64) checks EVERY unit of configs 1, 3 and 4 against the CUDA output and counts

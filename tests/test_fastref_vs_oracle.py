@@ -1,4 +1,4 @@
-"""Pins the harness-side numpy float64 pipeline (tests/fastref.py, SURVEY.md 8c-B "secondary full-coverage
+"""Pins the harness-side numpy float64 pipeline (fastref.py, SURVEY.md 8c-B "secondary full-coverage
 check") to the naive-DFT oracle on a subsample: E-field and amplitude <= 1e-12 relative, peak index equal,
 band limits equal. Only then may the GPU tests use it to cover EVERY unit of the big configs."""
 import numpy as np

@@ -1,6 +1,6 @@
 """Full-coverage GPU parity (SURVEY.md 8c-B "secondary full-coverage check", A9): EVERY unit of the big batch
 configs, in the launch configuration bench.py times (one call over the whole batch), against the harness-side
-numpy float64 pipeline of tests/fastref.py -- itself pinned to the oracle in tests/test_fastref_vs_oracle.py.
+numpy float64 pipeline of fastref.py -- itself pinned to the oracle in tests/test_fastref_vs_oracle.py.
 The oracle-sampled full-size tests stay in test_gpu_parity.py; this file adds the coverage the O(N K) oracle
 cannot afford, and reports how many peak indices were exact / near-tie +-1 / ambiguous (non-adjacent near-tie).
 
