@@ -80,7 +80,8 @@ def test_int16_input_matches_oracle(B, cfg, events, n_st, variant, kernel):
 
 
 # ------------------------------------------------------------------ row 4: spectral up-sampling
-@pytest.mark.parametrize("cfg,events,n_st,u", [(0, [0, 1], 7, 2), (0, [2], 7, 4), (1, [0], 6, 2), (3, [1], 3, 2), (0, [0], 3, 1)])
+@pytest.mark.parametrize("cfg,events,n_st,u", [(0, [0, 1], 7, 2), (0, [2], 7, 4), (1, [0], 6, 2), (3, [1], 3, 2), (0, [0], 3, 1),
+                                               (1, [0, 1], 124, 2)])   # N = 2048 x all 124 stations of an event
 def test_upsampled_matches_oracle(B, cfg, events, n_st, u):
     from oracle import aera_ext as ox
     wl = ai.WORKLOADS[cfg]

@@ -357,3 +357,60 @@ def test_scan_single_direction_and_station(B, orc):
         oamp, oidx, oe2 = orc.scan(wl.grid, H, wl.fs_hz, tr, dirs, want_env2=True)
         rep = compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx, oe2)
         assert_peaks(rep, wl.dtype)
+
+
+# ------------------------------------------------------------------ R8: exactly singular bins
+def _table_with_dead_cell(wl, j0):
+    """The seeded table with frequency nodes j0 and j0 + 1 set to zero: every DFT bin inside that frequency cell
+    interpolates between zero matrices, so its response is exactly singular (det == 0) at every direction."""
+    H = ai.pattern_table(wl.grid, wl.complex_dtype).copy()
+    H[..., j0:j0 + 2] = 0
+    return H
+
+
+@pytest.mark.parametrize("cfg,events,n_st,variant,kernel", [
+    (1, [0, 7], 9, 0, "unfold_w32"), (1, [0], 5, 1, "generic"), (0, [0, 1], 7, 0, "generic"),
+    (3, [0], 5, 0, "unfold_t4k_f64"), (4, [0], 2, 0, "unfold_long_f32")])
+def test_singular_bins_are_zeroed_like_the_oracle(B, orc, cfg, events, n_st, variant, kernel):
+    """DESIGN.md reading R8: a bin whose 2x2 response has det == 0 contributes nothing (E[k] = 0). The oracle does this
+    in oracle_solve2x2; here the CUDA branch runs on hardware against it, on every kernel family."""
+    wl = ai.WORKLOADS[cfg]
+    j0 = 6 if cfg != 4 else 50
+    H = _table_with_dead_cell(wl, j0)
+    f_lo = wl.grid.freq0_hz + j0 * wl.grid.dfreq_hz
+    k_dead = [k for k in range(1, wl.n_samples // 2) if f_lo <= k * wl.fs_hz / wl.n_samples <= f_lo + wl.grid.dfreq_hz]
+    assert len(k_dead) >= 2                                   # the cell really holds DFT bins of this (N, fs)
+    tr, dirs, _, _ = ai.make_batch(wl, events, n_stations=n_st)
+    dt = B.AERA_F32 if wl.dtype == "f32" else B.AERA_F64
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, dt), H)
+    old = B.aera_set_kernel_variant(variant)
+    try:
+        ef, amp, idx = B.aera_unfold_batch(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(dirs).cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        assert B.aera_last_kernel() == kernel
+    finally:
+        B.aera_set_kernel_variant(old)
+        pat.free()
+    efn = ef.cpu().numpy()
+    assert np.isfinite(efn).all() and np.isfinite(amp.cpu().numpy()).all()
+    # the dead bins carry no power in the output: compare with the live neighbours (fp32 round-off floor ~1e-7 of the band)
+    spec = np.abs(np.fft.rfft(efn.astype(np.float64), axis=-1))
+    live = spec[..., k_dead[0] - 12:k_dead[0] - 2].mean()
+    assert spec[..., k_dead].max() <= (1e-5 if wl.dtype == "f32" else 1e-12) * live, (spec[..., k_dead].max(), live)
+    check(wl, (efn, amp.cpu().numpy(), idx.cpu().numpy()), oracle_batch(orc, wl, H, tr, dirs))
+
+
+def test_singular_bins_in_the_scan(B, orc):
+    wl = ai.WORKLOADS[2]
+    H = _table_with_dead_cell(wl, 6)
+    ev = ai.make_event(wl, 0)
+    tr = np.ascontiguousarray(ev.traces[:9]); dirs = ai.scan_directions()[[0, 500, 3333, 7379]]
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        amp, idx = B.aera_scan_directions(pat, torch.from_numpy(tr).cuda(), torch.from_numpy(dirs).cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        assert B.aera_last_kernel() == "scan_w32"
+    finally:
+        pat.free()
+    oamp, oidx, oe2 = orc.scan(wl.grid, H, wl.fs_hz, tr, dirs, want_env2=True)
+    assert_peaks(compare_peaks(wl.dtype, amp.cpu().numpy(), idx.cpu().numpy(), oamp, oidx, oe2), wl.dtype)
