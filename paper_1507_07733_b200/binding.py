@@ -23,7 +23,7 @@ EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_worksp
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel", "aera_unfold_batch_multi", "aera_unfold_batch_i16",
            "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex", "aera_reconstruct_convergence",
-           "aera_unfold_batch_static", "aera_pattern_prepare", "aera_static_scratch_bytes")
+           "aera_unfold_batch_static", "aera_pattern_prepare", "aera_static_scratch_bytes", "aera_set_long_trace_l2_persist")
 
 
 class AeraError(RuntimeError):
@@ -79,6 +79,8 @@ def _load():
     lib.aera_set_kernel_variant.argtypes = [C.c_int]
     lib.aera_set_kernel_variant.restype = C.c_int
     lib.aera_launch_count.restype = C.c_ulonglong
+    lib.aera_set_long_trace_l2_persist.argtypes = [C.c_int]
+    lib.aera_set_long_trace_l2_persist.restype = C.c_int
     lib.aera_profile_enable.argtypes = [C.c_int]
     lib.aera_profile_enable.restype = C.c_int
     lib.aera_profile_read.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
@@ -168,6 +170,12 @@ def aera_launch_count() -> int:
 
 def aera_set_kernel_variant(variant: int) -> int:
     return int(_lib.aera_set_kernel_variant(int(variant)))
+
+
+def aera_set_long_trace_l2_persist(megabytes: int) -> int:
+    """Opt-in: let the N = 65536 kernel set the device's persisting-L2 carve-out (MB, clipped to the device maximum;
+    negative = leave the device's limit alone, the default). Returns the previous request."""
+    return int(_lib.aera_set_long_trace_l2_persist(int(megabytes)))
 
 
 def aera_last_kernel() -> str:

@@ -48,8 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(OBJ, src[:-3] + ".o")
-        extra = os.environ.get("AERA_NVCC_EXTRA", "").split()     # tuning only, e.g. -DAERA_SOLVE_UNROLL=4
-        cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         with open(os.path.join(OBJ, src[:-3] + ".ptxas.log"), "w") as f:
             f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)

@@ -152,6 +152,7 @@ cudaError_t launch_unfold_t4k(int dtype, const PlanDev &p, long n_events, int n_
 // ---- unfold_long_f32.cu: multi-pass kernel for N = 65536 fp32 through an L2-resident scratch (configs[4])
 bool long_f32_supported(int dtype, const PlanDev &p);
 size_t long_f32_scratch_bytes(const PlanDev &p);
+long set_long_persist_mb(long mb);   // aera_set_long_trace_l2_persist; returns the previous request
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
                                    void *amp, int32_t *idx, const void *minv, void *scratch, cudaStream_t s,
                                    const UnfoldExt &x = UnfoldExt());

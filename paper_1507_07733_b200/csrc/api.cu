@@ -367,6 +367,7 @@ aera_status_t aera_measure_alu_peak(int kind, int warps_per_sm, double *lane_fma
 const char *aera_version(void) { return "aera_unfold 0.1 (sm_100a)"; }
 unsigned long long aera_launch_count(void) { return g_launches.load(); }
 int aera_set_kernel_variant(int variant) { return g_variant.exchange(variant); }
+int aera_set_long_trace_l2_persist(int megabytes) { return (int)set_long_persist_mb(megabytes); }
 
 aera_status_t aera_pattern_upload(const aera_pattern_desc_t *desc, const void *H, int src_on_device,
                                   void *cuda_stream, aera_pattern_t **out)

@@ -2,8 +2,8 @@
 //
 // No tensor-core instruction is issued anywhere in this library (the path is not a contraction);
 // what the warp kernels need is a second place, besides shared memory, to park data that a lane
-// writes and later reads back ITSELF: the in-band spectrum between the two inverse transforms and
-// the even output samples until their odd neighbours exist. With the .32x32b shape of
+// writes and later reads back ITSELF: the in-band spectrum E between the two inverse transforms (one
+// per polarisation) and |z_theta|^2 of every sample until the phi pass adds |z_phi|^2 to it. With the .32x32b shape of
 // tcgen05.ld/st, thread t of warp w owns TMEM lane 32 (w % 4) + t and reads/writes consecutive
 // 32-bit columns of it: no bank conflicts by construction, a datapath separate from the LSU /
 // shared-memory crossbar (measured on B200, 8 warps/SM: STTM.x2 1.05, LDTM.x2 1.5 cycles per

@@ -468,6 +468,10 @@ static size_t long_stride(const PlanDev &p)
     const size_t C = (size_t)((p.k_hi >> 5) - (p.k_lo >> 5) + 1);
     return (2 * kYBytes + 2 * 32 * C * 8 + 2 * 16 * 1024 * 8 + 64 + 255) & ~(size_t)255;   // Y | E | parked pairs | U | per-CTA peaks
 }
+// megabytes of persisting-L2 carve-out requested through aera_set_long_trace_l2_persist; -1 = leave the device's limit alone
+static std::atomic<long> g_long_persist_mb{-1};
+long set_long_persist_mb(long mb) { return g_long_persist_mb.exchange(mb < 0 ? -1 : mb); }
+
 size_t long_f32_scratch_bytes(const PlanDev &p) { return long_max_clusters() * long_stride(p); }
 
 cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_stations, const void *traces, void *efield,
@@ -504,19 +508,22 @@ cudaError_t launch_unfold_long_f32(const PlanDev &p, long n_events, int n_statio
         }
         const long clusters = n_units < max_clusters ? n_units : max_clusters;
         // The scratch lines carry an evict_last policy, which holds only inside the persisting carve-out of the L2: without
-        // it a fifth of the scratch writes were evicted to DRAM before being overwritten (measured 1.83 MB of DRAM traffic
+        // one a fifth of the scratch writes are evicted to DRAM before being overwritten (measured 1.83 MB of DRAM traffic
         // per station against 1.05 MB algorithmic, 1.146 M stations/s; with a 79 MB carve-out 1.11 MB, 1.116 M stations/s;
-        // with 70 MB = the scratch size 1.23 MB, 1.135 M stations/s). Set once per process and device to the device maximum (79 MB
-        // on the B200); AERA_LONG_PERSIST_MB=<n> overrides, 0 leaves the limit alone.
-        static std::atomic<int> persist_done[kMaxDevices];      // the limit is a property of the device: once per device
-        if (slot < 0 || !persist_done[slot].exchange(1)) {
-            const char *ev = getenv("AERA_LONG_PERSIST_MB");
-            int mx = 0, dev = 0;
-            (void)cudaGetDevice(&dev);
-            (void)cudaDeviceGetAttribute(&mx, cudaDevAttrMaxPersistingL2CacheSize, dev);
-            size_t want = ev ? (size_t)atol(ev) << 20 : (size_t)mx;
-            if (want > (size_t)mx) want = (size_t)mx;
-            if (want > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) (void)cudaGetLastError();
+        // with 70 MB = the scratch size 1.23 MB, 1.135 M stations/s). The carve-out is device-wide state that belongs to
+        // the caller, so it is only touched on request: aera_set_long_trace_l2_persist (include/aera_unfold.h).
+        const long want_mb = g_long_persist_mb.load(std::memory_order_relaxed);
+        if (want_mb >= 0) {
+            static std::atomic<long> applied_mb[kMaxDevices];   // request last applied on each device, + 1 (0 = none yet)
+            if (slot < 0 || applied_mb[slot].load(std::memory_order_relaxed) != want_mb + 1) {
+                int mx = 0, dev = 0;
+                (void)cudaGetDevice(&dev);
+                (void)cudaDeviceGetAttribute(&mx, cudaDevAttrMaxPersistingL2CacheSize, dev);
+                size_t want = (size_t)want_mb << 20;
+                if (want > (size_t)mx) want = (size_t)mx;
+                if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) (void)cudaGetLastError();
+                if (slot >= 0) applied_mb[slot].store(want_mb + 1, std::memory_order_relaxed);
+            }
         }
         kern<<<(unsigned)(kLCluster * clusters), kLWarps * 32, smem, s>>>(q);
         return cudaGetLastError();

@@ -66,11 +66,8 @@ template <> struct T4k<float> {
     static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
 };
 // teams per CTA: 2 in fp64 (8 warps x 250 registers; a third team, 168 registers, gains nothing), 4 in fp32 (16 warps x 128)
-#ifndef AERA_T4K_TEAMS_F64
-#define AERA_T4K_TEAMS_F64 2
-#endif
 // (TW < 4: the same number of warps per CTA, i.e. 4 / TW times the teams)
-template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? AERA_T4K_TEAMS_F64 : 4;
+template <typename T> constexpr int kTeamsOf = sizeof(T) == 8 ? 2 : 4;
 constexpr int kPlaneBytes = 33 * 32 * 8;              // one warp's padded 32x32 transpose plane (sized for fp64)
 // region X of a team = TW planes (33 792 B at TW = 4): exchange buffer / transpose planes / mirror rows
 constexpr int kTabF64 = 2 * 1024 * 16;                // T (pass twiddles) + TQ (W_N^t, t < 1024)

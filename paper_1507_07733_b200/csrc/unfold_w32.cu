@@ -11,52 +11,42 @@
 //                   memory) the four real polyphase spectra separate, and
 //                   2 V_c[k] = F'_c0[k] + W_2048^k F'_c1[k]   (k < 1024 covers the whole band).
 //   a4 solve      : (E_theta, E_phi)[k] = Minv[event][k] (V_0, V_1)[k]; Minv = (1/N) H^-1 comes from
-//                   pattern.cu once per event, laid out as (theta, phi) pairs so E lands packed.
-//   a5 inverse    : the analytic spectrum is zero above N/2, so z[2m+s] = IFFT_1024(E[k] W_2048^{-sk}),
-//                   s = 0,1: two packed (theta, phi) transforms instead of two 2048-point ones.
-//                   The inverse is the forward routine with the re/im arrays swapped.
-//   a6 outputs    : e_p[n] = Re z_p[n] straight from registers; env^2 = |z_theta|^2 + |z_phi|^2 and a
-//                   running (max, lowest index) per lane, then a 5-step shuffle reduction.
+//                   pattern.cu once per event as two zero-padded planes (MINV_PACKED_PAD), so band-edge rows
+//                   multiply by zero instead of clamping and selecting. E goes to tensor memory.
+//   a5 inverse    : the analytic spectrum is zero above N/2, so (z_p[2m], z_p[2m+1]) = IFFT_1024 of
+//                   (E_p[k], E_p[k] W_2048^{-k}): ONE packed transform per polarisation whose two lanes
+//                   are the even and the odd samples (theta first, then phi), instead of two 2048-point
+//                   ones. The inverse is the forward routine with the re/im arrays swapped.
+//   a6 outputs    : Re z_p leaves the transform as the (even, odd) pair of an 8-byte store, straight from
+//                   registers. The theta pass parks |z_theta|^2 of both samples in tensor memory; the phi
+//                   pass adds |z_phi|^2 and keeps a running (max, lowest row) per lane and parity; the
+//                   warp argmax is two integer REDUX reductions (max of the float bits, then min index).
 //
-// Work distribution: CTA b owns the contiguous unit range [b n/G, (b+1) n/G); its 8 warps stride
+// Work distribution: CTA b owns the contiguous unit range [b n/G, (b+1) n/G); its twelve warps stride
 // through it. All stations of an event share Minv (one direction per event), so the
-// CTA keeps the current and the next event's Minv (18 KB each at configs[1]) in shared memory:
+// CTA keeps the current and the next event's Minv (20 KB each at configs[1]) in shared memory:
 // TMA bulk copies (cp.async.bulk + mbarrier) fill a two-slot ring; the last warp to leave event e
 // (shared-memory counter) issues the copy of event e+2 into the slot it vacates.
 //
 // HBM traffic per station: 16 KB read once (L2-prefetched one station ahead with
 // cp.async.bulk.prefetch.L2), 16 KB + 8 B written once, as (even, odd) sample pairs: 8 bytes per
-// lane, 256 contiguous bytes per store instruction, every 32-byte sector written once and in full.
+// lane, 256 contiguous bytes per store instruction, every 32-byte sector written once and in full,
+// with an L2 evict_first hint so the written lines do not push the prefetched traces out.
 //
 // Lane-private scratch lives in tensor memory (tmem.cuh), not in shared memory: the in-band
-// spectrum E (needed twice, s = 0 and 1) and Re z of the even samples (until the odd pass can pair
-// them up). That leaves one 10 KB transpose / mirror-exchange buffer per warp in shared memory, so
-// twelve warps (168 registers each) fit on an SM instead of eight: three warps per scheduler hide
-// each other's shared-memory and global-memory latencies.
+// spectrum E (read once per polarisation) and the parked |z_theta|^2. That leaves one 10 KB
+// transpose / mirror-exchange buffer per warp in shared memory, so twelve warps (168 registers each)
+// fit on an SM instead of eight: three warps per scheduler hide each other's shared-memory and
+// global-memory latencies.
 //
 // The in-band rows (bins k = lane + 32 row) are template parameters, so every per-row decision is
 // made at compile time; <10, 28> is configs[1] (k = 342..910), <0, 31> serves any other band.
 #include "w32_common.cuh"
 
-#ifndef AERA_W32_LD_POLICY
-#define AERA_W32_LD_POLICY 0
-#endif
-#ifndef AERA_W32_ABLATE
-#define AERA_W32_ABLATE 0   // timing experiments only (wrong results), bit mask: 1 no fft32, 2 no transposes, 4 no global loads/stores, 8 no pass twiddles, 16 no separation+solve, 32 no envelope/argmax
-#endif
-#ifndef AERA_PREFETCH_DIST
-#define AERA_PREFETCH_DIST 1
-#endif
-#ifndef AERA_FFT_LOOP_FORM
-#define AERA_FFT_LOOP_FORM 0
-#endif
-#ifndef AERA_SOLVE_UNROLL
-#define AERA_SOLVE_UNROLL 1
-#endif
 namespace aera {
 namespace {
 
-constexpr int kSolveUnroll = AERA_SOLVE_UNROLL;   // band rows of separate_solve in flight together
+constexpr int kSolveUnroll = 1;   // band rows of separate_solve in flight together (2 and 4 measured slower)
 
 struct W32Params {
     const void *traces;    // float [n_units][2][2048], or int16 ADC counts of the same shape (IN16)
@@ -233,9 +223,9 @@ unfold_w32_kernel(W32Params p)
             const float4 *MBu = MAu + KP;
             float *ef = HAS_EF ? p.efield + (size_t)u * 4 * kM : nullptr;
             float4 *sp = SPEC != 0 ? p.spectra + (size_t)u * G::kBandRows * 32 + lane : nullptr;
-            if (AERA_PREFETCH_DIST > 0 && lane == 0 && u + AERA_PREFETCH_DIST * kWarps < u1) {
-                if (SPEC != 2 && IN16) prefetch_l2_bulk(v16 + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(int16_t));
-                else if (SPEC != 2) prefetch_l2_bulk(v + (size_t)AERA_PREFETCH_DIST * kWarps * 4 * kM, 4 * kM * sizeof(float));
+            if (lane == 0 && u + kWarps < u1) {          // this warp's next station, one ahead (two ahead measured no better)
+                if (SPEC != 2 && IN16) prefetch_l2_bulk(v16 + (size_t)kWarps * 4 * kM, 4 * kM * sizeof(int16_t));
+                else if (SPEC != 2) prefetch_l2_bulk(v + (size_t)kWarps * 4 * kM, 4 * kM * sizeof(float));
                 else prefetch_l2_bulk(p.spectra + (size_t)(u + kWarps) * G::kBandRows * 32, G::kBandRows * 32 * sizeof(float4));
             }
 
@@ -244,20 +234,14 @@ unfold_w32_kernel(W32Params p)
                 // ---- a1: the station's two traces, read once, straight into FFT input order
                 static_for<0, 32>([&](auto jc) {
                     constexpr int j = decltype(jc)::value;
-                    if (AERA_W32_ABLATE & 4) { A[brev5(j)] = L::pack(lane * 0.5f, j); B[brev5(j)] = L::pack(j, lane); return; }
                     if (IN16) { // two ADC counts per 32-bit word: (v[2m], v[2m+1]); the counts-to-volts factors are in Minv
                         const int a = ld_stream_b32(v16 + 2 * (lane + 32 * j)), b = ld_stream_b32(v16 + 2 * kM + 2 * (lane + 32 * j));
                         A[brev5(j)] = L::pack((float)(short)(a & 0xffff), (float)(a >> 16));
                         B[brev5(j)] = L::pack((float)(short)(b & 0xffff), (float)(b >> 16));
                         return;
                     }
-#if AERA_W32_LD_POLICY
-                    A[brev5(j)] = ld_stream_b64_pol(v + 2 * (lane + 32 * j), pol_first);            // (v0[2m], v0[2m+1])
-                    B[brev5(j)] = ld_stream_b64_pol(v + 2 * kM + 2 * (lane + 32 * j), pol_first);   // (v1[2m], v1[2m+1])
-#else
                     A[brev5(j)] = ld_stream_b64(v + 2 * (lane + 32 * j));            // (v0[2m], v0[2m+1])
                     B[brev5(j)] = ld_stream_b64(v + 2 * kM + 2 * (lane + 32 * j));   // (v1[2m], v1[2m+1])
-#endif
                 });
             } else {
                 // ---- the forward spectrum of this station was stored by an earlier call: a4 straight away
@@ -279,38 +263,18 @@ unfold_w32_kernel(W32Params p)
             int t = SPEC == 2 ? 1 : 0;
 #pragma unroll 1
             for (;;) {
-#if AERA_FFT_LOOP_FORM == 1
-                // two passes of 32-point FFTs through ONE copy of their code: a bottom-tested loop whose body is the
-                // FFT followed by the conditional inter-pass work (a loop with the exit test in the middle is rotated
-                // by the compiler, which duplicates the 388-instruction FFT); the counter is opaque to the optimiser
-                int pass = 0;
-#pragma unroll 1
-                do {
-                    fft32<L>(A, B);
-                    asm volatile("" : "+r"(pass));
-                    if (pass == 0) {
-                        pass_twiddle(A, B, T, lane);
-                        transpose_plane(A, X, lane);
-                        transpose_plane(B, X, lane);
-                    }
-                    ++pass;
-                } while (pass < 2);
-#else
                 int second = 0;
                 asm volatile("" : "+r"(second));
 #pragma unroll 1
                 for (;;) {
-                    if (!(AERA_W32_ABLATE & 1)) fft32<L>(A, B);
+                    fft32<L>(A, B);
                     if (second) break;
-                    if (!(AERA_W32_ABLATE & 8)) pass_twiddle(A, B, T, lane);
-                    if (!(AERA_W32_ABLATE & 2)) {
+                    pass_twiddle(A, B, T, lane);
                     transpose_plane(A, X, lane);
                     transpose_plane(B, X, lane);
-                    }
                     second = 1;
                     asm volatile("" : "+r"(second));
                 }
-#endif
                 if (t == 2) break;
                 if (SPEC != 2 && t == 0) {
                     // ---- a2 done: publish the band rows and the rows that are somebody's bin 1024-k
@@ -324,7 +288,7 @@ unfold_w32_kernel(W32Params p)
                     // ---- separate channels, fold the two polyphase halves, a4: E = Minv V, one band
                     // row per iteration (a rolled loop: 40 instructions instead of 19 x 45), E goes to
                     // this lane's tensor-memory columns and is read back once per polarisation
-                    if (!(AERA_W32_ABLATE & 16)) separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MAu, MBu, p.k_lo, p.k_hi, lane, tstash, sp);
+                    separate_solve<G, MINV_SMEM, SPEC>(QA, QB, TS, MAu, MBu, p.k_lo, p.k_hi, lane, tstash, sp);
                     __syncwarp(); // all reads of the published rows done before the buffer is a transpose plane again
                     tmem_wait_st();
                 } else

@@ -24,12 +24,6 @@ __device__ __forceinline__ R ld_stream_b64(const void *p)
     asm volatile("ld.global.nc.L1::no_allocate.b64 %0, [%1];" : "=l"(r.v) : "l"(p));
     return r;
 }
-__device__ __forceinline__ R ld_stream_b64_pol(const void *p, unsigned long long pol)
-{
-    R r;
-    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(r.v) : "l"(p), "l"(pol));
-    return r;
-}
 __device__ __forceinline__ int ld_stream_b32(const void *p)
 {
     int r;
@@ -85,31 +79,20 @@ __device__ __forceinline__ void fft1024(R (&A)[32], R (&B)[32], R *X, const floa
     fft32<L>(A, B);
 }
 
-#ifndef AERA_W32_ABLATE
-#define AERA_W32_ABLATE 0   // timing experiments only, see unfold_w32.cu
-#endif
-#ifndef AERA_W32_ST_POLICY
-#define AERA_W32_ST_POLICY 1   // 1: E-field stores carry an L2 evict_first hint (the written lines do not push the L2-prefetched traces out)
-#endif
 __device__ __forceinline__ unsigned long long l2_policy_evict_first()
 {
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-// streamed output: the line leaves the L2 first
+// streamed output with an L2 evict_first hint: the written lines leave the L2 first instead of pushing the
+// L2-prefetched traces out
 __device__ __forceinline__ void st_global_b64_stream(void *p, R v, unsigned long long pol)
 {
-#if AERA_W32_ST_POLICY == 1
     asm volatile("st.global.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(p), "l"(v.v), "l"(pol) : "memory");
-#else
-    asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
-#endif
 }
 __device__ __forceinline__ void st_global_b64(void *p, R v)
 {
-    if ((AERA_W32_ABLATE & 4) && v.v != 0x123456789abcdefull) return;
-
     asm volatile("st.global.b64 [%0], %1;" ::"l"(p), "l"(v.v) : "memory");
 }
 
@@ -216,7 +199,7 @@ __device__ __forceinline__ void emit_theta(const R (&zr)[32], const R (&zi)[32],
 {
     static_for<0, 32>([&](auto bc) {
         constexpr int b = decltype(bc)::value;
-        if (HAS_EF && !(AERA_W32_ABLATE & 4)) st_global_b64_stream(ef + 2 * (lane + 32 * b), zr[b], pol);
+        if (HAS_EF) st_global_b64_stream(ef + 2 * (lane + 32 * b), zr[b], pol);
         R q = L::mul(zr[b], zr[b]);
         q = L::fma(zi[b], zi[b], q);
         tmem_st64(tpark + 2 * b, q.v);
@@ -245,7 +228,7 @@ __device__ __forceinline__ void emit_phi(const R (&zr)[32], const R (&zi)[32], i
         static_for<0, 8>([&](auto jc) {
             constexpr int j = decltype(jc)::value;
             constexpr int b = 8 * c + j;
-            if (HAS_EF && !(AERA_W32_ABLATE & 4)) st_global_b64_stream(ef + 2 * kM + 2 * (lane + 32 * b), zr[b], pol);
+            if (HAS_EF) st_global_b64_stream(ef + 2 * kM + 2 * (lane + 32 * b), zr[b], pol);
             R q; q.v = ev[j];
             q = L::fma(zr[b], zr[b], q);
             q = L::fma(zi[b], zi[b], q);
