@@ -785,6 +785,23 @@ def main():
                "matches_device_path": same, "copy_only_ms": t_copy * 1e3, "frac_of_copy_only": t_copy / t_e2e,
                "copy_only_note": "the step's H2D and D2H bytes copied concurrently on two streams with no kernel: the PCIe floor of this leg on this box"}
         del out_ef
+        # the same leg with the bytes cut where the method allows (the copies dominate): int16 ADC
+        # counts in (1/16 microvolt per count), peaks only out -- a second record, not the headline e2e
+        if wl.dtype == "f32" and world == 1:
+            g16 = (0.0625, 0.0625)
+            h16 = torch.clamp(torch.round(host_tr / g16[0]), -32768, 32767).to(torch.int16).pin_memory()
+            B.aera_unfold_batch_host_i16(pat, h16, g16, dirs_h, wl.fs_hz, peak_amp=out_amp, peak_idx=out_idx, want_efield=False)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            for _ in range(n_e2e):
+                B.aera_unfold_batch_host_i16(pat, h16, g16, dirs_h, wl.fs_hz, peak_amp=out_amp, peak_idx=out_idx, want_efield=False)
+            torch.cuda.synchronize()
+            t16 = (time.perf_counter() - t0) / n_e2e
+            e2e["int16_in_peaks_out"] = {"value": ne_h * wl.n_stations / t16, "unit": UNIT, "ms_per_step": t16 * 1e3, "steps": n_e2e,
+                                         "h2d_bytes_per_step": int(h16.numel() * 2 + dirs_h.numel() * 8),
+                                         "d2h_bytes_per_step": int(out_amp.numel() * 4 + out_idx.numel() * 4),
+                                         "api": "aera_unfold_batch_host_i16 (int16 counts in, efield_host = NULL)",
+                                         "peak_idx_equal_to_fp32_path": float((out_idx == d_idx[:ne_h].cpu()).float().mean())}
+            del h16
 
     # ---- CPU oracle baseline on the box's host cores (rank 0, N=1 only), bounded sample
     cpu = None

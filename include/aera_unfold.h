@@ -285,6 +285,22 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
                                      const double *dirs_host, void *efield_host, void *peak_amp_host,
                                      int32_t *peak_idx_host);
 
+/* aera_unfold_batch_host for int16 ADC counts (section 5, L79 and L83: the copies to and from the device, not
+ * the transforms, dominate the run time, so the lever of the host path is bytes). The traces cross PCIe as int16 (half
+ * the bytes of fp32) and are converted in the kernel exactly as aera_unfold_batch_i16 does; with efield_host == NULL
+ * only the peaks come back and no E-field is staged at all. Per station at n_samples = 2048: 8 192 B in + 8 B out
+ * (peaks only) or + 16 384 B (E-field), against 16 384 B + 16 392 B of the fp32 call.
+ *   traces_host      HOST [n_events][n_stations][2][n_samples] int16 (page-locked memory gives full PCIe speed)
+ *   counts_to_volts  HOST [2] double, one factor per channel
+ *   efield_host      HOST fp32 [n_events][n_stations][2][n_samples], or NULL (peaks only)
+ *   peak_amp_host / peak_idx_host  HOST fp32 / int32 [n_events][n_stations]
+ *   pattern          an AERA_F32 pattern
+ * SYNCHRONOUS; shares the pattern handle's staging buffers and streams with aera_unfold_batch_host (one call at a time
+ * per handle; the buffers grow on demand). Errors as aera_unfold_batch_host and aera_unfold_batch_i16. */
+aera_status_t aera_unfold_batch_host_i16(aera_pattern_t *pattern, int n_events, int n_stations, int n_samples, double fs_hz,
+                                         const int16_t *traces_host, const double *counts_to_volts, const double *dirs_host,
+                                         float *efield_host, float *peak_amp_host, int32_t *peak_idx_host);
+
 /*
  * Batch unfolding without a workspace and without any allocation (the operation of aera_unfold_batch; PAPER.md
  * section 2, L29 steps 3 + 4; section 5: keep the data on the device and the copies out of the loop).

@@ -22,6 +22,12 @@
  *   O7  Hilbert envelope sqrt(|z_theta|^2+|z_phi|^2), its maximum and the
  *       smallest index attaining it
  *
+ * The Fourier sums are accumulated PLAINLY, term after term in index order, not pairwise or compensated (SURVEY.md
+ * 8(c) suggested the latter): the error of a plain sum of n terms in double is at most about n * 1.1e-16 relative to
+ * the sum of magnitudes, i.e. <= 7e-12 at n = 65536 and <= 5e-13 at n = 4096 in the worst case and about sqrt(n) *
+ * 1.1e-16 (3e-14, 7e-15) in practice, well inside the 1e-11 tolerance of the fp64 parity tests; the numpy.fft pins
+ * (<= 1e-12) bound it from outside. Keeping the sum plain keeps the function readable against the definition.
+ *
  * Readings of the paper where it is silent or garbled are listed in DESIGN.md
  * (section "Readings"); the ones that matter here: envelope = modulus of the analytic
  * signal (R1), forward kernel e^{-2 pi i nk/N} unnormalised, inverse 1/N (R5),

@@ -23,7 +23,8 @@ EXPORTS = ("aera_pattern_upload", "aera_pattern_free", "aera_band", "aera_worksp
            "aera_scan_directions", "aera_unfold_batch_host", "aera_reconstruct_batch", "aera_fold_batch", "aera_pattern_set_band_filter", "aera_set_kernel_variant", "aera_launch_count",
            "aera_last_error", "aera_version", "aera_profile_enable", "aera_profile_read", "aera_measure_alu_peak", "aera_last_kernel", "aera_unfold_batch_multi", "aera_unfold_batch_i16",
            "aera_unfold_batch_upsampled", "aera_workspace_bytes_ex", "aera_reconstruct_convergence",
-           "aera_unfold_batch_static", "aera_pattern_prepare", "aera_static_scratch_bytes", "aera_set_long_trace_l2_persist")
+           "aera_unfold_batch_static", "aera_pattern_prepare", "aera_static_scratch_bytes", "aera_set_long_trace_l2_persist",
+           "aera_unfold_batch_host_i16")
 
 
 class AeraError(RuntimeError):
@@ -69,6 +70,8 @@ def _load():
     lib.aera_scan_directions.restype = C.c_int
     lib.aera_unfold_batch_host.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, vp, vp, vp]
     lib.aera_unfold_batch_host.restype = C.c_int
+    lib.aera_unfold_batch_host_i16.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, vp, C.POINTER(C.c_double), dp, vp, vp, vp]
+    lib.aera_unfold_batch_host_i16.restype = C.c_int
     lib.aera_reconstruct_batch.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, dp, C.c_int, dp, vp, vp, vp, vp, vp,
                                            vp, C.c_size_t, vp]
     lib.aera_reconstruct_batch.restype = C.c_int
@@ -449,4 +452,23 @@ def aera_unfold_batch_host(p: Pattern, traces: torch.Tensor, dirs: torch.Tensor,
     if peak_idx is None:
         peak_idx = torch.empty((E, S), dtype=torch.int32, pin_memory=pin)
     _check(_lib.aera_unfold_batch_host(p.handle, dt, E, S, N, fs_hz, _ptr(traces), _ptr(dirs), _ptr(efield), _ptr(peak_amp), _ptr(peak_idx)))
+    return efield, peak_amp, peak_idx
+
+
+def aera_unfold_batch_host_i16(p: Pattern, traces: torch.Tensor, counts_to_volts, dirs: torch.Tensor, fs_hz: float, efield=None,
+                               peak_amp=None, peak_idx=None, want_efield=True):
+    """HOST int16 ADC counts [E][S][2][N] (pinned for full speed). Synchronous. Returns fp32 (efield|None, peak_amp,
+    peak_idx) on the host; want_efield=False moves the peaks only."""
+    E, S, two, N = traces.shape
+    assert two == 2 and (not traces.is_cuda) and traces.is_contiguous() and traces.dtype == torch.int16
+    assert (not dirs.is_cuda) and dirs.dtype == torch.float64 and tuple(dirs.shape) == (E, 2) and dirs.is_contiguous()
+    pin = traces.is_pinned()
+    if efield is None and want_efield:
+        efield = torch.empty(traces.shape, dtype=torch.float32, pin_memory=pin)
+    if peak_amp is None:
+        peak_amp = torch.empty((E, S), dtype=torch.float32, pin_memory=pin)
+    if peak_idx is None:
+        peak_idx = torch.empty((E, S), dtype=torch.int32, pin_memory=pin)
+    g = (C.c_double * 2)(float(counts_to_volts[0]), float(counts_to_volts[1]))
+    _check(_lib.aera_unfold_batch_host_i16(p.handle, E, S, N, fs_hz, _ptr(traces), g, _ptr(dirs), _ptr(efield), _ptr(peak_amp), _ptr(peak_idx)))
     return efield, peak_amp, peak_idx

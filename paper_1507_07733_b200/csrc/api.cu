@@ -98,7 +98,7 @@ struct HostPipe { // staging for aera_unfold_batch_host
     int32_t *d_idx[2] = {nullptr, nullptr};
     double *d_dirs[2] = {nullptr, nullptr};
     void *d_ws[2] = {nullptr, nullptr};
-    size_t cap_units = 0, cap_trace_bytes = 0, cap_ws = 0, cap_events = 0;
+    size_t cap_units = 0, cap_in_bytes = 0, cap_out_bytes = 0, cap_ws = 0, cap_events = 0;
     bool ready = false;
 };
 
@@ -756,10 +756,11 @@ aera_status_t aera_reconstruct_convergence(const double *dirs_hist, int n_iter, 
     return AERA_OK;
 }
 
-aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
-                                     int n_samples, double fs_hz, const void *traces_host,
-                                     const double *dirs_host, void *efield_host, void *peak_amp_host,
-                                     int32_t *peak_idx_host)
+// aera_unfold_batch_host (in_i16 = 0) and aera_unfold_batch_host_i16 (in_i16 = 1: int16 ADC counts in, fp32 out)
+static aera_status_t host_impl(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                               int n_samples, double fs_hz, const void *traces_host, int in_i16, const double *counts_to_volts,
+                               const double *dirs_host, void *efield_host, void *peak_amp_host,
+                               int32_t *peak_idx_host)
 {
     aera_status_t st = check_common(pattern, dtype, n_stations, n_samples, fs_hz);
     if (st != AERA_OK) return st;
@@ -770,7 +771,8 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
 
     const size_t rb = real_bytes(dtype);
     const size_t unit_bytes = (size_t)2 * n_samples * rb;
-    const size_t event_bytes = unit_bytes * n_stations;
+    const size_t event_bytes = unit_bytes * n_stations;                                   // one event of E-field output
+    const size_t event_in_bytes = in_i16 ? (size_t)2 * n_samples * sizeof(int16_t) * n_stations : event_bytes;
     // chunk: ~64 MB of traces per stage (AERA_HOST_CHUNK_MB overrides, tuning only), at least one event
     static const size_t chunk_mb = [] { const char *e = getenv("AERA_HOST_CHUNK_MB"); const int v = e ? atoi(e) : 64; return (size_t)(v < 1 ? 1 : (v > 1024 ? 1024 : v)); }();
     long chunk_events = (long)((chunk_mb << 20) / event_bytes);
@@ -794,20 +796,22 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
     Plan *pl = nullptr;
     st = get_plan(pattern, n_samples, fs_hz, hp.st[1], &pl);
     if (st != AERA_OK) return st;
-    const size_t need_trace = (size_t)chunk_events * event_bytes;
+    const size_t need_in = (size_t)chunk_events * event_in_bytes;
+    const size_t need_out = efield_host ? (size_t)chunk_events * event_bytes : 0;          // peaks only: no E-field staging at all
     const size_t need_units = (size_t)chunk_events * n_stations;
     const size_t need_ws = ws_layout(AERA_OP_UNFOLD, dtype, n_samples, pl->dev.k_lo, pl->dev.K, chunk_events, n_stations).total;
-    if (need_trace > hp.cap_trace_bytes || need_units > hp.cap_units || need_ws > hp.cap_ws || (size_t)chunk_events > hp.cap_events) {
+    if (need_in > hp.cap_in_bytes || need_out > hp.cap_out_bytes || need_units > hp.cap_units || need_ws > hp.cap_ws || (size_t)chunk_events > hp.cap_events) {
+        const size_t new_in = need_in > hp.cap_in_bytes ? need_in : hp.cap_in_bytes, new_out = need_out > hp.cap_out_bytes ? need_out : hp.cap_out_bytes;
         cudaDeviceSynchronize();
         for (int i = 0; i < 2; ++i) {
             cudaFree(hp.d_in[i]); cudaFree(hp.d_out[i]); cudaFree(hp.d_amp[i]); cudaFree(hp.d_idx[i]); cudaFree(hp.d_dirs[i]); cudaFree(hp.d_ws[i]);
             hp.d_in[i] = hp.d_out[i] = hp.d_amp[i] = hp.d_ws[i] = nullptr; hp.d_idx[i] = nullptr; hp.d_dirs[i] = nullptr;
-            bool ok = cudaMalloc(&hp.d_in[i], need_trace) == cudaSuccess && cudaMalloc(&hp.d_out[i], need_trace) == cudaSuccess &&
+            bool ok = cudaMalloc(&hp.d_in[i], new_in) == cudaSuccess && (new_out == 0 || cudaMalloc(&hp.d_out[i], new_out) == cudaSuccess) &&
                       cudaMalloc(&hp.d_amp[i], need_units * 8) == cudaSuccess && cudaMalloc((void **)&hp.d_idx[i], need_units * 4) == cudaSuccess &&
                       cudaMalloc((void **)&hp.d_dirs[i], (size_t)chunk_events * 16) == cudaSuccess && cudaMalloc(&hp.d_ws[i], need_ws) == cudaSuccess;
-            if (!ok) { (void)cudaGetLastError(); hp.cap_trace_bytes = hp.cap_units = hp.cap_ws = hp.cap_events = 0; return fail(AERA_ERR_ALLOC, "cudaMalloc of host-pipeline staging buffers failed"); }
+            if (!ok) { (void)cudaGetLastError(); hp.cap_in_bytes = hp.cap_out_bytes = hp.cap_units = hp.cap_ws = hp.cap_events = 0; return fail(AERA_ERR_ALLOC, "cudaMalloc of host-pipeline staging buffers failed"); }
         }
-        hp.cap_trace_bytes = need_trace; hp.cap_units = need_units; hp.cap_ws = need_ws; hp.cap_events = (size_t)chunk_events;
+        hp.cap_in_bytes = new_in; hp.cap_out_bytes = new_out; hp.cap_units = need_units; hp.cap_ws = need_ws; hp.cap_events = (size_t)chunk_events;
     }
 
     const unsigned char *tin = static_cast<const unsigned char *>(traces_host);
@@ -824,12 +828,17 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
             if ((e = cudaStreamWaitEvent(hp.st[0], hp.ev_k[b], 0)) != cudaSuccess) return drained(cuda_fail(e, "stream wait"));
             if ((e = cudaStreamWaitEvent(hp.st[1], hp.ev_out[b], 0)) != cudaSuccess) return drained(cuda_fail(e, "stream wait"));
         }
-        if ((e = cudaMemcpyAsync(hp.d_in[b], tin + (size_t)done * event_bytes, (size_t)ne * event_bytes, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return drained(cuda_fail(e, "H2D traces"));
+        if ((e = cudaMemcpyAsync(hp.d_in[b], tin + (size_t)done * event_in_bytes, (size_t)ne * event_in_bytes, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return drained(cuda_fail(e, "H2D traces"));
         if ((e = cudaMemcpyAsync(hp.d_dirs[b], dirs_host + 2 * done, (size_t)ne * 16, cudaMemcpyHostToDevice, hp.st[0])) != cudaSuccess) return drained(cuda_fail(e, "H2D dirs"));
         cudaEventRecord(hp.ev_in[b], hp.st[0]);
         cudaStreamWaitEvent(hp.st[1], hp.ev_in[b], 0);
-        st = aera_unfold_batch(pattern, dtype, (int)ne, n_stations, n_samples, fs_hz, hp.d_in[b], hp.d_dirs[b],
-                               efield_host ? hp.d_out[b] : nullptr, hp.d_amp[b], hp.d_idx[b], hp.d_ws[b], hp.cap_ws, hp.st[1]);
+        if (in_i16)
+            st = aera_unfold_batch_i16(pattern, (int)ne, n_stations, n_samples, fs_hz, static_cast<const int16_t *>(hp.d_in[b]), counts_to_volts,
+                                       hp.d_dirs[b], efield_host ? static_cast<float *>(hp.d_out[b]) : nullptr, static_cast<float *>(hp.d_amp[b]),
+                                       hp.d_idx[b], hp.d_ws[b], hp.cap_ws, hp.st[1]);
+        else
+            st = aera_unfold_batch(pattern, dtype, (int)ne, n_stations, n_samples, fs_hz, hp.d_in[b], hp.d_dirs[b],
+                                   efield_host ? hp.d_out[b] : nullptr, hp.d_amp[b], hp.d_idx[b], hp.d_ws[b], hp.cap_ws, hp.st[1]);
         if (st != AERA_OK) return drained(st);
         cudaEventRecord(hp.ev_k[b], hp.st[1]);
         cudaStreamWaitEvent(hp.st[2], hp.ev_k[b], 0);
@@ -843,6 +852,25 @@ aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_e
     for (int i = 0; i < 3; ++i)
         if ((e = cudaStreamSynchronize(hp.st[i])) != cudaSuccess) return cuda_fail(e, "host pipeline synchronise");
     return AERA_OK;
+}
+
+aera_status_t aera_unfold_batch_host(aera_pattern_t *pattern, int dtype, int n_events, int n_stations,
+                                     int n_samples, double fs_hz, const void *traces_host,
+                                     const double *dirs_host, void *efield_host, void *peak_amp_host,
+                                     int32_t *peak_idx_host)
+{
+    return host_impl(pattern, dtype, n_events, n_stations, n_samples, fs_hz, traces_host, 0, nullptr, dirs_host, efield_host,
+                     peak_amp_host, peak_idx_host);
+}
+
+aera_status_t aera_unfold_batch_host_i16(aera_pattern_t *pattern, int n_events, int n_stations, int n_samples, double fs_hz,
+                                         const int16_t *traces_host, const double *counts_to_volts, const double *dirs_host,
+                                         float *efield_host, float *peak_amp_host, int32_t *peak_idx_host)
+{
+    if (!counts_to_volts || !std::isfinite(counts_to_volts[0]) || !std::isfinite(counts_to_volts[1]))
+        return fail(AERA_ERR_INVALID_ARG, "counts_to_volts must point to two finite factors (host memory)");
+    return host_impl(pattern, AERA_F32, n_events, n_stations, n_samples, fs_hz, traces_host, 1, counts_to_volts, dirs_host, efield_host,
+                     peak_amp_host, peak_idx_host);
 }
 
 } // extern "C"

@@ -228,3 +228,40 @@ def test_multi_pattern_ids_out_of_range_are_clamped(B, cfg, n_st, kernel):
     finally:
         for p in pats:
             p.free()
+
+
+def test_host_pipeline_int16_matches_device_path_and_oracle(B):
+    """aera_unfold_batch_host_i16: int16 counts from host memory through the chunked 3-stream pipeline. Bit-equal to the
+    device call aera_unfold_batch_i16 (the same kernels on the same chunks' data), against the int16 oracle on a sample,
+    peaks-only mode (no E-field staged or copied), and the staging buffers shared with the fp32 host call grow as needed."""
+    from oracle import aera_ext as ox
+    wl = ai.WORKLOADS[1]
+    H = ai.pattern_table(wl.grid, wl.complex_dtype)
+    E, S = 70, 124                                        # 70 events x 124 stations x 16 KB of E-field = 139 MB: three 64 MB chunks
+    tr, dirs, _, _ = ai.make_batch_parallel(wl, range(10))
+    tr = np.ascontiguousarray(np.tile(tr, (7, 1, 1, 1))); dirs = np.ascontiguousarray(np.tile(dirs, (7, 1)))
+    g = (0.0625, 0.05)
+    counts = np.stack([np.clip(np.round(tr[:, :, c] / g[c]), -32768, 32767) for c in (0, 1)], axis=2).astype(np.int16)
+    c_h = torch.from_numpy(counts).pin_memory(); d_h = torch.from_numpy(dirs).pin_memory()
+    pat = B.aera_pattern_upload(B.make_desc(wl.grid, B.AERA_F32), H)
+    try:
+        _, amp_p, idx_p = B.aera_unfold_batch_host_i16(pat, c_h, g, d_h, wl.fs_hz, want_efield=False)     # peaks only first: no d_out yet
+        ef_h, amp_h, idx_h = B.aera_unfold_batch_host_i16(pat, c_h, g, d_h, wl.fs_hz)                    # staging grows for the E-field
+        ef_d, amp_d, idx_d = B.aera_unfold_batch_i16(pat, c_h.cuda(), g, d_h.cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        assert torch.equal(ef_h, ef_d.cpu()) and torch.equal(amp_h, amp_d.cpu()) and torch.equal(idx_h, idx_d.cpu())
+        assert torch.equal(amp_p, amp_h) and torch.equal(idx_p, idx_h)
+        t_h = torch.from_numpy(tr[:3]).pin_memory()                                                      # the fp32 host call on the same handle
+        ef_f, amp_f, idx_f = B.aera_unfold_batch_host(pat, t_h, d_h[:3].clone().pin_memory(), wl.fs_hz)
+        ef_g, amp_g, idx_g = B.aera_unfold_batch(pat, t_h.cuda(), d_h[:3].cuda(), wl.fs_hz)
+        torch.cuda.synchronize()
+        assert torch.equal(ef_f, ef_g.cpu()) and torch.equal(idx_f, idx_g.cpu())
+        with pytest.raises(B.AeraError):
+            B.aera_unfold_batch_host_i16(pat, c_h, (float("nan"), 1.0), d_h, wl.fs_hz)
+    finally:
+        pat.free()
+    ev, st = np.array([0, 9, 33, 69]), np.array([0, 57, 123])
+    sel = counts[ev][:, st].reshape(-1, 2, wl.n_samples)
+    ref = ox.unfold_batch_i16(wl.grid, H, wl.fs_hz, sel, g, np.repeat(dirs[ev], len(st), axis=0), want_env2=True)
+    _check(wl, compare("f32", ef_h.numpy()[ev][:, st].reshape(-1, 2, wl.n_samples), amp_h.numpy()[ev][:, st].ravel(),
+                       idx_h.numpy()[ev][:, st].ravel(), ref), "host int16 pipeline")
