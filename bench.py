@@ -220,8 +220,11 @@ def run_sizes(args):
     hbm, src = load_peaks()
     grid = ai.WORKLOADS[0].grid
     fs = args.fs_mhz * 1e6 if args.fs_mhz > 0 else 200e6
-    for dtype, N in (("f32", 1024), ("f64", 1024), ("f32", 2048), ("f64", 2048), ("f32", 4096), ("f64", 4096),
-                     ("f32", 8192), ("f64", 8192), ("f32", 16384)):
+    sizes = (("f32", 1024), ("f64", 1024), ("f32", 2048), ("f64", 2048), ("f32", 4096), ("f64", 4096),
+             ("f32", 8192), ("f64", 8192), ("f32", 16384))
+    if args.small:   # the sizes below the register-resident kernels: both variants are the generic kernels there (configs[0] is N = 256)
+        sizes = tuple((dt, n) for n in (64, 128, 256, 512) for dt in ("f32", "f64"))
+    for dtype, N in sizes:
         td = torch.float32 if dtype == "f32" else torch.float64
         H = ai.pattern_table(grid, np.complex64 if dtype == "f32" else np.complex128)
         pat = B.aera_pattern_upload(B.make_desc(grid, B.AERA_F32 if dtype == "f32" else B.AERA_F64), H)
@@ -583,6 +586,7 @@ def main():
     ap.add_argument("--fold", action="store_true", help="time the on-device forward model (aera_fold_batch) on the config's shapes")
     ap.add_argument("--peaks", action="store_true", help="measure and print the device's ALU issue peaks (packed fp32, fp32, fp64) and exit")
     ap.add_argument("--sizes", action="store_true", help="throughput of the dispatched and the generic kernels at N = 1024 / 2048 / 4096, fp32 and fp64 (one JSON line each) and exit")
+    ap.add_argument("--small", action="store_true", help="with --sizes: N = 64 / 128 / 256 / 512 instead (the generic kernels; configs[0] is N = 256)")
     ap.add_argument("--i16", action="store_true", help="int16 ADC-count input (aera_unfold_batch_i16): 24 584 algorithmic bytes per unit at configs[1]")
     ap.add_argument("--upsample", type=int, default=1, help="spectral up-sampling factor (aera_unfold_batch_upsampled; the E-field output is this many times larger)")
     ap.add_argument("--patterns", type=int, default=1, help="number of resident antenna-pattern tables, stations assigned round-robin (aera_unfold_batch_multi)")
